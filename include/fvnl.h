@@ -1,0 +1,145 @@
+/* fvnl.h -- C ABI of the B200-native finite-volume step for nonlinear thermoviscous acoustics.
+ *
+ * Implements the per-time-step 2-D high-resolution finite-volume update of arXiv 1311.3004
+ * (Velasco-Segura & Rendon), Sections II-III.  "PAPER.md:<line>" cites /root/reference/PAPER.md.
+ *
+ *   conservation system (19a,b) in the dimensionless form (21)-(23)
+ *   fractional steps: x-sweep (24) -> y-sweep (25) -> source step (26)
+ *   wave-propagation update (27), fluctuations (28),(29), MC-limited F~ (30)
+ *   Roe matrix of the arithmetic-mean primitive state, eigenvalues (32)-(34)
+ *   CFL number nu and lagged time-step control towards nu_W
+ *   boundary cells: analytic (41), focused source (43), zero-order extrapolation,
+ *   reflecting border
+ *
+ * General conventions
+ *   - Every function returns an int status (0 = FVNL_OK) unless noted.  No exceptions, no aborts, no output.
+ *   - The library runs on the CUDA device that is current when fvnl_create is called and on the CUDA stream
+ *     passed to it.  There is NO CPU fallback: without a usable device fvnl_create returns FVNL_ECUDA.
+ *   - The caller owns every buffer it passes.  The library copies in / out and never keeps a caller pointer,
+ *     except `workspace` (fvnl_create), which must stay valid until fvnl_destroy.
+ *   - State = the paper's dimensionless conserved vector q of (22), PAPER.md:133:
+ *         q1 = rho/rho0,  q2 = q1*u/c0,  q3 = q1*v/c0        (equilibrium: 1, 0, 0)
+ *     as three separate contiguous planes of nx*ny values, index = j*nx + i, i = x index (fastest).
+ *   - Pointers named `*_dev_or_host` are device pointers when `on_device != 0`, host pointers otherwise.
+ *   - SI units at the boundary (m, s, Hz); only lambda = c0 dt/dx, kappa = delta dt/dx^2 and beta enter the update.
+ */
+#ifndef FVNL_H
+#define FVNL_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fvnl_ctx fvnl_ctx;
+
+/* Host-side status codes (returned as such) and sticky device flags (OR-ed together, returned by fvnl_step). */
+enum {
+    FVNL_OK = 0,
+    FVNL_EARG = 1,      /* bad argument                                                    */
+    FVNL_EALLOC = 2,    /* workspace too small / allocation failed                         */
+    FVNL_ECUDA = 3,     /* CUDA runtime error or no device                                 */
+    FVNL_ESTATE = 4,    /* call order (e.g. step before set_state)                         */
+    FVNL_ECFL = 16,     /* a step ran with nu > 1 or kappa_x + kappa_y > 1/2 */
+    FVNL_ENONREAL = 32, /* square-root argument of (32),(33) negative        */
+    FVNL_ENONPOS = 64,  /* q1 <= 0 met in a primitive conversion                            */
+    FVNL_ENAN = 128     /* NaN met                                                          */
+};
+
+/* Medium of (19): small-signal sound speed [m/s], equilibrium density [kg/m^3], coefficient of nonlinearity
+ * beta = 1 + B/(2A), sound diffusivity delta [m^2/s] (18). */
+typedef struct { double c0, rho0, beta, delta; } fvnl_medium;
+
+/* Edge kinds.  PERIODIC must be set on both sides of an axis.  REFLECT mirrors the interior and negates the
+ * normal momentum (the paper's reflecting bottom border).  EXTRAP is zero-order extrapolation
+ * ("simplified absorbing").  SOURCE prescribes the ghost cells analytically (below). */
+enum { FVNL_BC_EXTRAP = 0, FVNL_BC_PERIODIC = 1, FVNL_BC_REFLECT = 2, FVNL_BC_SOURCE = 3 };
+enum { FVNL_SIDE_XLO = 0, FVNL_SIDE_XHI = 1, FVNL_SIDE_YLO = 2, FVNL_SIDE_YHI = 3 };
+
+/* Source shapes.  With d = (coordinate of the ghost cell's centre along the edge, from the low corner) - centre_m,
+ * lambda_w = c0/freq_hz, and, when 0 < focus_m < inf,  R = sqrt(d^2 + focus_m^2):
+ *     tau = freq_hz*(t + t0_s) + d^2/(2*focus_m*lambda_w)          [periods]      tau of (43)
+ *     SINE  : g = amp*sin(2 pi tau) for tau >= 0, else 0           (plane piston = SINE with focus_m <= 0)
+ *     PACKET: g = amp*sin(2 pi tau)*exp(-(tau/4)^10)               (43d), PAPER.md:417 (exponent sign: DESIGN.md A13)
+ *     q1 = 1 + g ; inward-normal momentum = g*focus_m/R ; along-edge momentum = -g*d/R      (43a-c)
+ *     (focus_m <= 0 or infinite: plane wave, tau has no d term, normal momentum = g, along-edge momentum = 0).
+ *   Both ghost layers of the edge take the same values (they sample (43) at the edge, A14).  Cells with
+ *   |d| > half_aperture_m (> 0) behave as FVNL_BC_EXTRAP; half_aperture_m <= 0: the whole edge.
+ *     TANH  : q1 = 1 - amp*tanh(steep*(x - c0*(t + t0_s))), q2 = q1 - 1, q3 = 0        (41)
+ *   with x = the x coordinate of the ghost cell's OWN centre measured from the x-lo edge (negative in the x-lo
+ *   ghosts): (41) is a field, the same on whichever side it is attached to.  steep [1/m].
+ *   Sources are evaluated at t_n, the time at the start of the step. */
+enum { FVNL_SRC_SINE = 0, FVNL_SRC_PACKET = 1, FVNL_SRC_TANH = 2 };
+typedef struct {
+    int shape;
+    double amp;             /* dimensionless: u0/c0 = p'/(rho0 c0^2)                                   */
+    double freq_hz;
+    double focus_m;         /* F of (43); <= 0 or inf: plane wave                                      */
+    double centre_m;        /* aperture centre along the edge, from the low corner                     */
+    double half_aperture_m; /* a of PAPER.md:405; <= 0: whole edge                                     */
+    double t0_s;
+    double steep;           /* TANH only                                                               */
+} fvnl_source;
+
+/* Bytes of device memory the context needs for an nx x ny grid (second state buffer, clock, reduction slots).
+ * precision: 64 (fp32 is not built in this round -> 0 is returned for anything else). */
+size_t fvnl_workspace_bytes(int nx, int ny, int precision);
+
+/* Create a context.  nx, ny >= 4; dx, dy, c0, rho0 > 0; beta >= 1; delta >= 0; precision = 64.
+ * cuda_stream: a cudaStream_t (NULL = default stream); all work of this context is issued on it.
+ * workspace: DEVICE memory of at least fvnl_workspace_bytes() bytes, 256-byte aligned, owned by the caller (e.g. a
+ * torch tensor) and kept alive until fvnl_destroy; or NULL, then the library cudaMallocs it itself.
+ * Initial state: equilibrium (1,0,0), all edges EXTRAP, t = 0.
+ * Errors: FVNL_EARG, FVNL_EALLOC (workspace_bytes too small / cudaMalloc failed), FVNL_ECUDA. */
+int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy, const fvnl_medium* medium, int precision,
+                void* cuda_stream, void* workspace_dev, size_t workspace_bytes);
+
+/* Release the context (and its workspace if the library allocated it).  NULL is allowed. */
+void fvnl_destroy(fvnl_ctx* ctx);
+
+/* Set the rule for one edge.  src is read for FVNL_BC_SOURCE only (copied).  FVNL_EARG on bad side/kind/shape or
+ * missing src.  A lone PERIODIC side is reported by fvnl_step (FVNL_EARG). */
+int fvnl_set_bc(fvnl_ctx* ctx, int side, int kind, const fvnl_source* src_or_null);
+
+/* Copy a state in (three planes of nx*ny doubles).  Resets the sticky flags and the lagged maximum M (the next
+ * CFL-mode step starts with the pre-pass), keeps t.  Asynchronous on the stream for device input; for host input
+ * the buffers may be reused when the call returns. */
+int fvnl_set_state(fvnl_ctx* ctx, const void* q1_dev_or_host, const void* q2_dev_or_host,
+                   const void* q3_dev_or_host, int on_device);
+
+/* Set the clock: simulation time t [s] and the lagged maximum M [1/m] of the previous step.
+ * last_M <= 0: recompute M by the pre-pass on the current state at the next CFL-mode step.
+ * (t, M) from fvnl_get_info + the state from fvnl_get_state restart a run bit-exactly. */
+int fvnl_set_clock(fvnl_ctx* ctx, double t_s, double last_M);
+
+/* Advance nsteps time steps.  Each step: ghost rule -> x-sweep (24) -> y-sweep (25) -> source step (26), (27)-(34).
+ *   mode 0: value = dt [s], fixed.
+ *   mode 1: value = nu_W; dt_n = nu_W/(c0*M_{n-1}), M = max over all x-interfaces of |s|/dx and y-interfaces of
+ *           |s|/dy met during the previous step; first step: a pre-pass over the current state.
+ *           No step is rejected; a step that ran with nu_n = c0*dt_n*M_n > 1 sets FVNL_ECFL.
+ * The steps are queued on the stream without host synchronisation (dt lives on the device); the call then reads
+ * back 64 bytes {flags, t, dt, M, steps} and returns the OR of the sticky device flags (0 = clean).  With flags
+ * set the state is undefined but readable.
+ * Errors: FVNL_EARG (nsteps < 0, value <= 0, bad mode, lone PERIODIC, mode 0 with delta*dt*(1/dx^2+1/dy^2) > 1/2),
+ * FVNL_ECUDA. */
+int fvnl_step(fvnl_ctx* ctx, long nsteps, double value, int mode);
+
+/* Copy the current state out (three planes of nx*ny doubles).  Synchronises the stream for host output. */
+int fvnl_get_state(fvnl_ctx* ctx, void* q1_dev_or_host, void* q2_dev_or_host, void* q3_dev_or_host, int on_device);
+
+/* Clock and step statistics after the last fvnl_step: time [s], last dt [s], CFL number of the last step
+ * nu = c0*dt*M, last M [1/m], number of steps taken since fvnl_create.  Any pointer may be NULL.  Synchronises. */
+int fvnl_get_info(fvnl_ctx* ctx, double* t_s, double* last_dt_s, double* last_cfl, double* last_M,
+                  long* steps_done);
+
+/* Number of kernels this context has launched so far (sweeps, pre-pass, packing); for bench accounting. */
+long fvnl_kernel_launches(const fvnl_ctx* ctx);
+
+/* Text for a status code or flag word (static storage). */
+const char* fvnl_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FVNL_H */

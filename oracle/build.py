@@ -1,0 +1,25 @@
+"""Build the CPU oracle shared library (test infrastructure, not the product).
+
+g++ -O2 -ffp-contract=off -fopenmp: no fast-math, no FMA contraction, so every formula of
+fvnl_oracle.cpp rounds exactly as written.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "fvnl_oracle.cpp")
+LIB = os.path.join(HERE, "libfvnl_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+        return LIB
+    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
+           "-shared", "-fPIC", "-o", LIB, SRC]
+    subprocess.run(cmd, check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv))
