@@ -133,6 +133,15 @@ int fvnl_get_state(fvnl_ctx* ctx, void* q1_dev_or_host, void* q2_dev_or_host, vo
 int fvnl_get_info(fvnl_ctx* ctx, double* t_s, double* last_dt_s, double* last_cfl, double* last_M,
                   long* steps_done);
 
+/* Kernel selection.  FVNL_KERNEL_DEFAULT: the fused one-pass step kernel (the product path).  FVNL_KERNEL_UNFUSED:
+ * the three-pass form (x-sweep, y-sweep, source step as separate kernels through HBM; allocates one more
+ * y-extended state with cudaMalloc on first use) -- a measured comparison point for "what fusion buys" and an
+ * independently structured second implementation for cross-checks.  Same results up to rounding.
+ * FVNL_OPT_ROWS_PER_BLOCK: rows one thread block of the fused kernel marches over (0 = automatic). */
+enum { FVNL_OPT_KERNEL = 0, FVNL_OPT_ROWS_PER_BLOCK = 1 };
+enum { FVNL_KERNEL_DEFAULT = 0, FVNL_KERNEL_UNFUSED = 1 };
+int fvnl_set_option(fvnl_ctx* ctx, int option, int value);
+
 /* Number of kernels this context has launched so far (sweeps, pre-pass, packing); for bench accounting. */
 long fvnl_kernel_launches(const fvnl_ctx* ctx);
 

@@ -1,0 +1,354 @@
+// fvnl.cu -- C-ABI library of the B200-native finite-volume step of arXiv 1311.3004 (include/fvnl.h).
+//
+// Host side: context, argument checks, launch sequence.  All arithmetic of the path runs in the kernels of
+// fvnl_fused.cuh (default) or fvnl_unfused.cuh (opt-in comparison path); there is no CPU fallback.
+// Build: paper_1311_3004_b200/build.py (nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo).
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/fvnl.h"
+#include "fvnl_unfused.cuh"
+
+using namespace fvnl;
+
+// ---------------------------------------------------------------------------------------------------------------
+// Clock kernels (one thread).  PAPER.md:275-279, readings A7, A8.
+// mode 0: value = dt; mode 1: value = nu_W, dt = nu_W / (c0 M_prev).
+__global__ void k_clock_begin(Grid g, Clock* c, double value, int mode) {
+    const double dt = (mode == 1) ? __ddiv_rn(value, __dmul_rn(g.c0, c->Mprev)) : value;
+    c->dt = dt;
+    c->lamx = __ddiv_rn(__dmul_rn(g.c0, dt), g.dx);
+    c->lamy = __ddiv_rn(__dmul_rn(g.c0, dt), g.dy);
+    c->kapx = __ddiv_rn(__dmul_rn(g.delta, dt), __dmul_rn(g.dx, g.dx));
+    c->kapy = __ddiv_rn(__dmul_rn(g.delta, dt), __dmul_rn(g.dy, g.dy));
+    if (__dadd_rn(c->kapx, c->kapy) > 0.5) c->flags |= F_ECFL;
+    if (!(dt > 0.0) || not_finite(dt)) c->flags |= F_ENAN;
+    c->sx_bits = 0ull;
+    c->sy_bits = 0ull;
+}
+
+// End of step n (M_n, nu_n, t) fused with the beginning of step n+1 when `more` is set.
+__global__ void k_clock_end(Grid g, Clock* c, double value, int mode, int more) {
+    const double sx = __longlong_as_double((long long)c->sx_bits), sy = __longlong_as_double((long long)c->sy_bits);
+    const double M = fmax(__ddiv_rn(sx, g.dx), __ddiv_rn(sy, g.dy));
+    c->last_dt = c->dt;
+    c->last_cfl = __dmul_rn(__dmul_rn(g.c0, c->dt), M);
+    if (c->last_cfl > 1.0) c->flags |= F_ECFL;
+    c->Mprev = M;
+    c->t = __dadd_rn(c->t, c->dt);
+    c->steps += 1;
+    if (more) {
+        const double dt = (mode == 1) ? __ddiv_rn(value, __dmul_rn(g.c0, M)) : value;
+        c->dt = dt;
+        c->lamx = __ddiv_rn(__dmul_rn(g.c0, dt), g.dx);
+        c->lamy = __ddiv_rn(__dmul_rn(g.c0, dt), g.dy);
+        c->kapx = __ddiv_rn(__dmul_rn(g.delta, dt), __dmul_rn(g.dx, g.dx));
+        c->kapy = __ddiv_rn(__dmul_rn(g.delta, dt), __dmul_rn(g.dy, g.dy));
+        if (__dadd_rn(c->kapx, c->kapy) > 0.5) c->flags |= F_ECFL;
+        if (!(dt > 0.0) || not_finite(dt)) c->flags |= F_ENAN;
+        c->sx_bits = 0ull;
+        c->sy_bits = 0ull;
+    }
+}
+
+// O7 pre-pass: M of the current state = max |s|/h over the x-interfaces of G_x(Q) and the y-interfaces of G_y(Q)
+// that touch an interior cell (first step of CFL mode).  Thread (i, j) owns its low interfaces (+ the high ones on
+// the last column / row).
+__global__ void __launch_bounds__(256) k_prepass(Grid g, Clock* clk, const double* __restrict__ q1,
+                                                 const double* __restrict__ q2, const double* __restrict__ q3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y;
+    const double t = clk->t, b2 = 2.0 * (g.beta - 1.0);
+    int flags = 0;
+    double sx = 0.0, sy = 0.0;
+    if (i < g.nx) {
+        const Q3 c = load_ext(g, q1, q2, q3, i, j, t);
+        const CellX cx = make_cell(c.q1, c.q2, c.q3, flags), cy = make_cell(c.q1, c.q3, c.q2, flags);
+        {
+            const Q3 w = load_ext(g, q1, q2, q3, i - 1, j, t);
+            sx = max_speed(riemann_x(make_cell(w.q1, w.q2, w.q3, flags), cx, b2, flags));
+            if (i == g.nx - 1) {
+                const Q3 e = load_ext(g, q1, q2, q3, i + 1, j, t);
+                sx = fmax(sx, max_speed(riemann_x(cx, make_cell(e.q1, e.q2, e.q3, flags), b2, flags)));
+            }
+        }
+        {
+            const Q3 s = load_ext(g, q1, q2, q3, i, j - 1, t);
+            sy = max_speed(riemann_x(make_cell(s.q1, s.q3, s.q2, flags), cy, b2, flags));
+            if (j == g.ny - 1) {
+                const Q3 n = load_ext(g, q1, q2, q3, i, j + 1, t);
+                sy = fmax(sy, max_speed(riemann_x(cy, make_cell(n.q1, n.q3, n.q2, flags), b2, flags)));
+            }
+        }
+    }
+    block_max_to(&clk->sx_bits, sx);
+    __syncthreads();
+    block_max_to(&clk->sy_bits, sy);
+    block_flags_to(&clk->flags, flags);
+}
+
+__global__ void k_fill(double* p, size_t n, double v) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = v;
+}
+
+__global__ void k_prepass_end(Grid g, Clock* c) {
+    const double sx = __longlong_as_double((long long)c->sx_bits), sy = __longlong_as_double((long long)c->sy_bits);
+    c->Mprev = fmax(__ddiv_rn(sx, g.dx), __ddiv_rn(sy, g.dy));
+    c->sx_bits = 0ull;
+    c->sy_bits = 0ull;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+struct fvnl_ctx {
+    Grid g;
+    int device;
+    cudaStream_t stream;
+    size_t n;                   // nx*ny
+    void* ws;                   // workspace base
+    bool own_ws;
+    Clock* clk;                 // device clock
+    double* buf[2][3];          // two state buffers (ping-pong); cur = index of the current state
+    int cur;
+    double* star[3];            // unfused path only: Q* on the y-extended mesh, allocated on first use
+    Clock* host_clk;            // pinned
+    Clock snap;                 // last read-back
+    bool have_state;
+    bool need_prepass;
+    int kernel;                 // FVNL_KERNEL_*
+    long launches;
+};
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static const size_t CLOCK_BYTES = 256;
+
+extern "C" size_t fvnl_workspace_bytes(int nx, int ny, int precision) {
+    if (nx < 4 || ny < 4 || precision != 64) return 0;
+    const size_t plane = align_up((size_t)nx * ny * sizeof(double), 256);
+    return CLOCK_BYTES + 6 * plane;
+}
+
+#define CK(call)                                         \
+    do {                                                 \
+        cudaError_t e_ = (call);                         \
+        if (e_ != cudaSuccess) { (void)cudaGetLastError(); return FVNL_ECUDA; } \
+    } while (0)
+
+extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy, const fvnl_medium* m, int precision,
+                           void* cuda_stream, void* workspace, size_t workspace_bytes) {
+    if (!out) return FVNL_EARG;
+    *out = nullptr;
+    if (nx < 4 || ny < 4 || !(dx > 0) || !(dy > 0) || !m || !(m->c0 > 0) || !(m->rho0 > 0) || !(m->beta >= 1) ||
+        !(m->delta >= 0) || precision != 64)
+        return FVNL_EARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { (void)cudaGetLastError(); return FVNL_ECUDA; }
+    fvnl_ctx* c = new (std::nothrow) fvnl_ctx();
+    if (!c) return FVNL_EALLOC;
+    std::memset(c, 0, sizeof(*c));
+    if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return FVNL_ECUDA; }
+    c->g.nx = nx; c->g.ny = ny; c->g.dx = dx; c->g.dy = dy;
+    c->g.c0 = m->c0; c->g.beta = m->beta; c->g.delta = m->delta;
+    for (int s = 0; s < 4; ++s) c->g.side[s].kind = BC_EXTRAP;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->n = (size_t)nx * ny;
+    const size_t need = fvnl_workspace_bytes(nx, ny, precision);
+    if (workspace) {
+        if (workspace_bytes < need || ((size_t)workspace & 255)) { delete c; return FVNL_EALLOC; }
+        c->ws = workspace;
+    } else {
+        if (cudaMalloc(&c->ws, need) != cudaSuccess) { (void)cudaGetLastError(); delete c; return FVNL_EALLOC; }
+        c->own_ws = true;
+    }
+    const size_t plane = align_up(c->n * sizeof(double), 256);
+    char* p = (char*)c->ws;
+    c->clk = (Clock*)p;
+    p += CLOCK_BYTES;
+    for (int b = 0; b < 2; ++b)
+        for (int k = 0; k < 3; ++k) { c->buf[b][k] = (double*)p; p += plane; }
+    if (cudaMallocHost((void**)&c->host_clk, sizeof(Clock)) != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (c->own_ws) cudaFree(c->ws);
+        delete c;
+        return FVNL_EALLOC;
+    }
+    std::memset(&c->snap, 0, sizeof(Clock));
+    bool ok = cudaMemsetAsync(c->clk, 0, CLOCK_BYTES, c->stream) == cudaSuccess;
+    // equilibrium state (1, 0, 0)
+    ok = ok && cudaMemsetAsync(c->buf[0][1], 0, plane, c->stream) == cudaSuccess;
+    ok = ok && cudaMemsetAsync(c->buf[0][2], 0, plane, c->stream) == cudaSuccess;
+    k_fill<<<592, 256, 0, c->stream>>>(c->buf[0][0], c->n, 1.0);
+    ok = ok && cudaGetLastError() == cudaSuccess;
+    c->launches = 1;
+    c->have_state = true;
+    c->need_prepass = true;
+    c->kernel = FVNL_KERNEL_DEFAULT;
+    if (!ok) { (void)cudaGetLastError(); fvnl_destroy(c); return FVNL_ECUDA; }
+    *out = c;
+    return FVNL_OK;
+}
+
+extern "C" void fvnl_destroy(fvnl_ctx* c) {
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    for (int k = 0; k < 3; ++k)
+        if (c->star[k]) cudaFree(c->star[k]);
+    if (c->host_clk) cudaFreeHost(c->host_clk);
+    if (c->own_ws && c->ws) cudaFree(c->ws);
+    (void)cudaGetLastError();
+    delete c;
+}
+
+extern "C" int fvnl_set_bc(fvnl_ctx* c, int side, int kind, const fvnl_source* s) {
+    if (!c || side < 0 || side > 3 || kind < 0 || kind > 3) return FVNL_EARG;
+    Side d;
+    std::memset(&d, 0, sizeof(d));
+    d.kind = kind;
+    if (kind == BC_SOURCE) {
+        if (!s || s->shape < 0 || s->shape > 2) return FVNL_EARG;
+        if (s->shape != SRC_TANH && !(s->freq_hz > 0)) return FVNL_EARG;
+        d.shape = s->shape; d.amp = s->amp; d.freq_hz = s->freq_hz; d.focus_m = s->focus_m; d.centre_m = s->centre_m;
+        d.half_aperture_m = s->half_aperture_m; d.t0_s = s->t0_s; d.steep = s->steep;
+    }
+    c->g.side[side] = d;
+    return FVNL_OK;
+}
+
+extern "C" int fvnl_set_option(fvnl_ctx* c, int option, int value) {
+    if (!c) return FVNL_EARG;
+    if (option == FVNL_OPT_KERNEL) {
+        if (value != FVNL_KERNEL_DEFAULT && value != FVNL_KERNEL_UNFUSED) return FVNL_EARG;
+        c->kernel = value;
+        return FVNL_OK;
+    }
+    return FVNL_EARG;
+}
+
+extern "C" int fvnl_set_state(fvnl_ctx* c, const void* q1, const void* q2, const void* q3, int on_device) {
+    if (!c || !q1 || !q2 || !q3) return FVNL_EARG;
+    const void* src[3] = {q1, q2, q3};
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(c->buf[c->cur][k], src[k], c->n * sizeof(double), kind, c->stream));
+    // reset sticky flags and the lagged maximum, keep t (and the step counter)
+    c->snap.flags = 0;
+    c->snap.Mprev = 0.0;
+    c->snap.sx_bits = c->snap.sy_bits = 0ull;
+    *c->host_clk = c->snap;
+    CK(cudaMemcpyAsync(c->clk, c->host_clk, sizeof(Clock), cudaMemcpyHostToDevice, c->stream));
+    if (!on_device) CK(cudaStreamSynchronize(c->stream));
+    else CK(cudaStreamSynchronize(c->stream));   // host_clk staging buffer is reused by later calls
+    c->have_state = true;
+    c->need_prepass = true;
+    return FVNL_OK;
+}
+
+extern "C" int fvnl_set_clock(fvnl_ctx* c, double t_s, double last_M) {
+    if (!c || !(t_s == t_s)) return FVNL_EARG;
+    CK(cudaStreamSynchronize(c->stream));
+    c->snap.t = t_s;
+    c->snap.Mprev = last_M > 0.0 ? last_M : 0.0;
+    *c->host_clk = c->snap;
+    CK(cudaMemcpyAsync(c->clk, c->host_clk, sizeof(Clock), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    c->need_prepass = !(last_M > 0.0);
+    return FVNL_OK;
+}
+
+static int ensure_star(fvnl_ctx* c) {
+    if (c->star[0]) return FVNL_OK;
+    const size_t bytes = (size_t)(c->g.ny + 4) * c->g.nx * sizeof(double);
+    for (int k = 0; k < 3; ++k)
+        if (cudaMalloc((void**)&c->star[k], bytes) != cudaSuccess) { (void)cudaGetLastError(); return FVNL_EALLOC; }
+    return FVNL_OK;
+}
+
+static int read_clock(fvnl_ctx* c) {
+    CK(cudaMemcpyAsync(c->host_clk, c->clk, sizeof(Clock), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    c->snap = *c->host_clk;
+    return FVNL_OK;
+}
+
+extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
+    if (!c || nsteps < 0 || !(value > 0.0) || (mode != 0 && mode != 1)) return FVNL_EARG;
+    if (!c->have_state) return FVNL_ESTATE;
+    const Grid& g = c->g;
+    for (int ax = 0; ax < 2; ++ax)
+        if ((g.side[2 * ax].kind == BC_PERIODIC) != (g.side[2 * ax + 1].kind == BC_PERIODIC)) return FVNL_EARG;
+    if (mode == 0 && g.delta * value / (g.dx * g.dx) + g.delta * value / (g.dy * g.dy) > 0.5) return FVNL_EARG;
+    if (nsteps == 0) return c->snap.flags;
+    cudaStream_t st = c->stream;
+    const dim3 blk(256), grd((g.nx + 255) / 256, g.ny);
+    if (mode == 1 && c->need_prepass) {
+        k_prepass<<<grd, blk, 0, st>>>(g, c->clk, c->buf[c->cur][0], c->buf[c->cur][1], c->buf[c->cur][2]);
+        k_prepass_end<<<1, 1, 0, st>>>(g, c->clk);
+        c->launches += 2;
+        c->need_prepass = false;
+    }
+    k_clock_begin<<<1, 1, 0, st>>>(g, c->clk, value, mode);
+    c->launches += 1;
+    if (c->kernel == FVNL_KERNEL_UNFUSED) {
+        const int rc = ensure_star(c);
+        if (rc) return rc;
+    }
+    for (long n = 0; n < nsteps; ++n) {
+        double** a = c->buf[c->cur];
+        double** b = c->buf[c->cur ^ 1];
+        {
+            const dim3 grdx((g.nx + 255) / 256, g.ny + 4);
+            k_xsweep_unfused<<<grdx, blk, 0, st>>>(g, c->clk, a[0], a[1], a[2], c->star[0], c->star[1], c->star[2]);
+            k_ysweep_unfused<<<grd, blk, 0, st>>>(g, c->clk, c->star[0], c->star[1], c->star[2], b[0], b[1], b[2]);
+            k_source_unfused<<<grd, blk, 0, st>>>(g, c->clk, b[0], b[1], b[2], a[0], a[1], a[2]);
+            c->launches += 3;
+            // result is back in `a`: cur unchanged
+        }
+        k_clock_end<<<1, 1, 0, st>>>(g, c->clk, value, mode, n + 1 < nsteps ? 1 : 0);
+        c->launches += 1;
+    }
+    CK(cudaGetLastError());
+    const int rc = read_clock(c);
+    if (rc) return rc;
+    // M of the last step is known: a following CFL-mode call continues without a pre-pass (restartable, P10)
+    return c->snap.flags;
+}
+
+extern "C" int fvnl_get_state(fvnl_ctx* c, void* q1, void* q2, void* q3, int on_device) {
+    if (!c || !q1 || !q2 || !q3) return FVNL_EARG;
+    if (!c->have_state) return FVNL_ESTATE;
+    void* dst[3] = {q1, q2, q3};
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(dst[k], c->buf[c->cur][k], c->n * sizeof(double), kind, c->stream));
+    if (!on_device) CK(cudaStreamSynchronize(c->stream));
+    return FVNL_OK;
+}
+
+extern "C" int fvnl_get_info(fvnl_ctx* c, double* t_s, double* last_dt_s, double* last_cfl, double* last_M, long* steps) {
+    if (!c) return FVNL_EARG;
+    const int rc = read_clock(c);
+    if (rc) return rc;
+    if (t_s) *t_s = c->snap.t;
+    if (last_dt_s) *last_dt_s = c->snap.last_dt;
+    if (last_cfl) *last_cfl = c->snap.last_cfl;
+    if (last_M) *last_M = c->snap.Mprev;
+    if (steps) *steps = (long)c->snap.steps;
+    return FVNL_OK;
+}
+
+extern "C" long fvnl_kernel_launches(const fvnl_ctx* c) { return c ? c->launches : 0; }
+
+extern "C" const char* fvnl_strerror(int code) {
+    switch (code) {
+        case FVNL_OK: return "ok";
+        case FVNL_EARG: return "bad argument";
+        case FVNL_EALLOC: return "workspace too small or allocation failed";
+        case FVNL_ECUDA: return "CUDA error or no device";
+        case FVNL_ESTATE: return "call order: no state set";
+        default: break;
+    }
+    if (code & ~(FVNL_ECFL | FVNL_ENONREAL | FVNL_ENONPOS | FVNL_ENAN)) return "unknown code";
+    static thread_local char buf[96];
+    std::snprintf(buf, sizeof(buf), "device flags:%s%s%s%s", (code & FVNL_ECFL) ? " CFL>1" : "",
+                  (code & FVNL_ENONREAL) ? " non-real-eigenvalue" : "", (code & FVNL_ENONPOS) ? " q1<=0" : "",
+                  (code & FVNL_ENAN) ? " NaN" : "");
+    return buf;
+}

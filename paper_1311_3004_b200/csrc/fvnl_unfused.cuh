@@ -1,0 +1,154 @@
+// fvnl_unfused.cuh -- three-pass form of the step: x-sweep, y-sweep and source step as separate kernels, one thread
+// per cell, every thread solving the Riemann problems of its own 5-cell stencil (4x redundant).  It exists as the
+// measured "what fusion buys" comparison point (144 B/cell-update of HBM traffic) and as the
+// second, independently structured GPU implementation the fused kernel is cross-checked against bit by bit in
+// tests/.  The product default is the fused kernel (fvnl_fused.cuh); this path is opt-in (FVNL_KERNEL_UNFUSED).
+#pragma once
+#include "fvnl_bc.cuh"
+
+namespace fvnl {
+
+// Block-wide max of non-negative doubles -> atomicMax on the bit pattern (order preserving for x >= 0).
+__device__ __forceinline__ void block_max_to(unsigned long long* slot, double v) {
+    unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long other = __shfl_xor_sync(0xffffffffu, b, o);
+        b = other > b ? other : b;
+    }
+    __shared__ unsigned long long red[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) red[wid] = b;
+    __syncthreads();
+    if (wid == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        b = lane < nw ? red[lane] : 0ull;
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long other = __shfl_xor_sync(0xffffffffu, b, o);
+            b = other > b ? other : b;
+        }
+        if (lane == 0 && b != 0ull) atomicMax(slot, b);
+    }
+}
+
+__device__ __forceinline__ void block_flags_to(int* slot, int f) {
+    f = __reduce_or_sync(0xffffffffu, f);
+    if ((threadIdx.x & 31) == 0 && f) atomicOr(slot, f);
+}
+
+// (27) for the middle cell of a 5-cell stencil c[0..4] in x-form.  Returns Q* of c[2]; `sl` / `sr`: the speeds of
+// its left / right interface for M.
+__device__ __forceinline__ Q3 sweep_cell(const CellX c[5], double lam, double beta2m2, double& sl, double& sr, int& flags) {
+    Waves w[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) w[k] = riemann_x(c[k], c[k + 1], beta2m2, flags);
+    Flux3 F[2];
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+        const Waves& k = w[1 + e];
+        const Waves& lo = w[e];
+        const Waves& hi = w[2 + e];
+        const bool u1 = k.s1 > 0.0, u2 = k.s2 > 0.0, u3 = k.s3 > 0.0;      // upwind interface is k-1
+        F[e] = interface_flux(k, u1 ? lo.al1 : hi.al1, u1 ? lo.s1 : hi.s1, u1 ? lo.r31 : hi.r31,
+                              u2 ? lo.al2 : hi.al2, u2 ? lo.s2 : hi.s2, u2 ? lo.r32 : hi.r32,
+                              u3 ? lo.al3 : hi.al3, lam);
+    }
+    sl = max_speed(w[1]);
+    sr = max_speed(w[2]);
+    Q3 o;
+    o.q1 = fma(-lam, F[0].p1 + F[1].m1, c[2].q1);
+    o.q2 = fma(-lam, F[0].p2 + F[1].m2, c[2].q2);
+    o.q3 = fma(-lam, F[0].p3 + F[1].m3, c[2].q3);
+    if (not_finite(o.q1) || not_finite(o.q2) || not_finite(o.q3)) flags |= F_ENAN;
+    return o;
+}
+
+// O2: x-sweep (24) of the y-extended mesh, rows -2 .. ny+1 -> star (row r stored at r+2).  grid.y = ny+4.
+__global__ void __launch_bounds__(256) k_xsweep_unfused(Grid g, Clock* clk, const double* __restrict__ q1,
+                                                        const double* __restrict__ q2, const double* __restrict__ q3,
+                                                        double* __restrict__ s1, double* __restrict__ s2,
+                                                        double* __restrict__ s3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = (int)blockIdx.y - 2;
+    const double t = clk->t, lam = clk->lamx;
+    int flags = 0;
+    double smax = 0.0;
+    if (i < g.nx) {
+        CellX c[5];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const Q3 q = load_ext(g, q1, q2, q3, i - 2 + k, r, t);
+            c[k] = make_cell(q.q1, q.q2, q.q3, flags);
+        }
+        double sl, sr;
+        const Q3 o = sweep_cell(c, lam, 2.0 * (g.beta - 1.0), sl, sr, flags);
+        const size_t idx = (size_t)(r + 2) * g.nx + i;
+        s1[idx] = o.q1; s2[idx] = o.q2; s3[idx] = o.q3;
+        if (r >= 0 && r < g.ny) smax = fmax(sl, sr); else flags = 0;      // ghost rows do not enter M (O5)
+    }
+    block_max_to(&clk->sx_bits, smax);
+    block_flags_to(&clk->flags, flags);
+}
+
+// O3: y-sweep (25) of star with positions 2 and 3 switched -> o1..o3 (interior).
+__global__ void __launch_bounds__(256) k_ysweep_unfused(Grid g, Clock* clk, const double* __restrict__ s1,
+                                                        const double* __restrict__ s2, const double* __restrict__ s3,
+                                                        double* __restrict__ o1, double* __restrict__ o2,
+                                                        double* __restrict__ o3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y;
+    const double lam = clk->lamy;
+    int flags = 0;
+    double smax = 0.0;
+    if (i < g.nx) {
+        CellX c[5];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const size_t idx = (size_t)(j + k) * g.nx + i;               // star row (j-2+k) is stored at j+k
+            c[k] = make_cell(s1[idx], s3[idx], s2[idx], flags);
+        }
+        double sl, sr;
+        const Q3 o = sweep_cell(c, lam, 2.0 * (g.beta - 1.0), sl, sr, flags);
+        const size_t idx = (size_t)j * g.nx + i;
+        o1[idx] = o.q1; o2[idx] = o.q3; o3[idx] = o.q2;
+        smax = fmax(sl, sr);
+    }
+    block_max_to(&clk->sy_bits, smax);
+    block_flags_to(&clk->flags, flags);
+}
+
+// O4: source step (26): q^m += kap_x d2x(q^m/q^1) + kap_y d2y(q^m/q^1), m = 2, 3 (readings A1, A2).
+__global__ void __launch_bounds__(256) k_source_unfused(Grid g, const Clock* clk, const double* __restrict__ a1,
+                                                        const double* __restrict__ a2, const double* __restrict__ a3,
+                                                        double* __restrict__ o1, double* __restrict__ o2,
+                                                        double* __restrict__ o3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y;
+    if (i >= g.nx) return;
+    const double t = clk->t, kx = clk->kapx, ky = clk->kapy;
+    auto at = [&](int ii, int jj) {
+        const size_t idx = (size_t)jj * g.nx + ii;
+        Q3 c; c.q1 = a1[idx]; c.q2 = a2[idx]; c.q3 = a3[idx];
+        return c;
+    };
+    const Q3 c = at(i, j);
+    Q3 w, e, s, n;
+    const bool px = g.side[SIDE_XLO].kind == BC_PERIODIC, py = g.side[SIDE_YLO].kind == BC_PERIODIC;
+    if (i > 0) w = at(i - 1, j);
+    else w = ghost_of(g, SIDE_XLO, px ? at(g.nx - 1, j) : c, (j + 0.5) * g.dy, -0.5 * g.dx, t);
+    if (i < g.nx - 1) e = at(i + 1, j);
+    else e = ghost_of(g, SIDE_XHI, px ? at(0, j) : c, (j + 0.5) * g.dy, (g.nx + 0.5) * g.dx, t);
+    if (j > 0) s = at(i, j - 1);
+    else s = ghost_of(g, SIDE_YLO, py ? at(i, g.ny - 1) : c, (i + 0.5) * g.dx, (i + 0.5) * g.dx, t);
+    if (j < g.ny - 1) n = at(i, j + 1);
+    else n = ghost_of(g, SIDE_YHI, py ? at(i, 0) : c, (i + 0.5) * g.dx, (i + 0.5) * g.dx, t);
+    const double rc = 1.0 / c.q1, rw = 1.0 / w.q1, re = 1.0 / e.q1, rs = 1.0 / s.q1, rn = 1.0 / n.q1;
+    const double z2 = c.q2 * rc, z3 = c.q3 * rc;
+    const double lx2 = (e.q2 * re + w.q2 * rw) - 2.0 * z2, ly2 = (n.q2 * rn + s.q2 * rs) - 2.0 * z2;
+    const double lx3 = (e.q3 * re + w.q3 * rw) - 2.0 * z3, ly3 = (n.q3 * rn + s.q3 * rs) - 2.0 * z3;
+    const size_t idx = (size_t)j * g.nx + i;
+    o1[idx] = c.q1;
+    o2[idx] = fma(ky, ly2, fma(kx, lx2, c.q2));
+    o3[idx] = fma(ky, ly3, fma(kx, lx3, c.q3));
+}
+
+}  // namespace fvnl
