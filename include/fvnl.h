@@ -138,9 +138,19 @@ int fvnl_get_info(fvnl_ctx* ctx, double* t_s, double* last_dt_s, double* last_cf
  * y-extended state with cudaMalloc on first use) -- a measured comparison point for "what fusion buys" and an
  * independently structured second implementation for cross-checks.  Same results up to rounding.
  * FVNL_OPT_ROWS_PER_BLOCK: rows one thread block of the fused kernel marches over (0 = automatic). */
-enum { FVNL_OPT_KERNEL = 0, FVNL_OPT_ROWS_PER_BLOCK = 1 };
+enum { FVNL_OPT_KERNEL = 0, FVNL_OPT_ROWS_PER_BLOCK = 1, FVNL_OPT_KERNEL_TIMING = 2 };
 enum { FVNL_KERNEL_DEFAULT = 0, FVNL_KERNEL_UNFUSED = 1 };
 int fvnl_set_option(fvnl_ctx* ctx, int option, int value);
+
+/* Per-kernel device time, for the roofline figures of bench.py.  With FVNL_OPT_KERNEL_TIMING set to 1, fvnl_step
+ * records a CUDA event pair on the context's stream around every launch of the kernels below (no host
+ * synchronisation is added; at most 65536 launches are kept between two reads).  fvnl_get_kernel_time
+ * synchronises the stream, returns the summed device time [ms] and the number of launches of kernel `which`
+ * since the previous read of that kernel, and resets both.  FVNL_EARG on a bad `which`.
+ *   FVNL_TIMED_STEP  : the fused one-pass step kernel (default path)
+ *   FVNL_TIMED_XSWEEP / _YSWEEP / _SOURCE : the three kernels of the unfused path */
+enum { FVNL_TIMED_STEP = 0, FVNL_TIMED_XSWEEP = 1, FVNL_TIMED_YSWEEP = 2, FVNL_TIMED_SOURCE = 3, FVNL_TIMED_KINDS = 4 };
+int fvnl_get_kernel_time(fvnl_ctx* ctx, int which, double* total_ms, long* launches);
 
 /* Number of kernels this context has launched so far (sweeps, pre-pass, packing); for bench accounting. */
 long fvnl_kernel_launches(const fvnl_ctx* ctx);

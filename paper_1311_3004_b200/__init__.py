@@ -25,7 +25,8 @@ SINE, PACKET, TANH = 0, 1, 2
 XLO, XHI, YLO, YHI = 0, 1, 2, 3
 OK, EARG, EALLOC, ECUDA, ESTATE = 0, 1, 2, 3, 4
 ECFL, ENONREAL, ENONPOS, ENAN = 16, 32, 64, 128
-OPT_KERNEL, OPT_ROWS_PER_BLOCK = 0, 1
+OPT_KERNEL, OPT_ROWS_PER_BLOCK, OPT_KERNEL_TIMING = 0, 1, 2
+TIMED_STEP, TIMED_XSWEEP, TIMED_YSWEEP, TIMED_SOURCE = 0, 1, 2, 3
 KERNEL_DEFAULT, KERNEL_UNFUSED = 0, 1
 
 
@@ -70,6 +71,7 @@ def lib():
         L.fvnl_step.argtypes = [_vp, C.c_long, C.c_double, C.c_int]
         L.fvnl_get_state.argtypes = [_vp, _vp, _vp, _vp, C.c_int]
         L.fvnl_get_info.argtypes = [_vp] + [C.POINTER(C.c_double)] * 4 + [C.POINTER(C.c_long)]
+        L.fvnl_get_kernel_time.argtypes = [_vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_long)]
         L.fvnl_kernel_launches.restype = C.c_long
         L.fvnl_kernel_launches.argtypes = [_vp]
         L.fvnl_strerror.restype = C.c_char_p
@@ -123,6 +125,12 @@ def fvnl_get_info(h):
     n = C.c_long()
     rc = lib().fvnl_get_info(h, C.byref(t), C.byref(dt), C.byref(cfl), C.byref(M), C.byref(n))
     return rc, dict(t=t.value, dt=dt.value, cfl=cfl.value, M=M.value, steps=n.value)
+
+
+def fvnl_get_kernel_time(h, which):
+    ms, n = C.c_double(), C.c_long()
+    rc = lib().fvnl_get_kernel_time(h, int(which), C.byref(ms), C.byref(n))
+    return rc, ms.value, n.value
 
 
 def fvnl_kernel_launches(h):
@@ -227,6 +235,12 @@ class Solver:
         rc, d = fvnl_get_info(self._h)
         self._check("fvnl_get_info", rc)
         return d
+
+    def kernel_time(self, which):
+        """(summed device ms, launches) of one timed kernel since the last read (needs OPT_KERNEL_TIMING = 1)."""
+        rc, ms, n = fvnl_get_kernel_time(self._h, which)
+        self._check("fvnl_get_kernel_time", rc)
+        return ms, n
 
     def kernel_launches(self):
         return fvnl_kernel_launches(self._h)

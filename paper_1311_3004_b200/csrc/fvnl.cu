@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "../../include/fvnl.h"
 #include "fvnl_unfused.cuh"
@@ -117,7 +118,44 @@ struct fvnl_ctx {
     bool need_prepass;
     int kernel;                 // FVNL_KERNEL_*
     long launches;
+    // opt-in per-kernel timing (FVNL_OPT_KERNEL_TIMING): event pairs around the sweep kernels, resolved on demand
+    bool timing;
+    struct Span { int id; cudaEvent_t a, b; };
+    std::vector<Span>* spans;
+    double span_ms[FVNL_TIMED_KINDS];
+    long span_n[FVNL_TIMED_KINDS];
 };
+
+static const size_t MAX_SPANS = 1 << 16;
+
+// Event pair around one kernel launch (timing on only).
+struct SpanGuard {
+    fvnl_ctx* c;
+    cudaEvent_t b;
+    SpanGuard(fvnl_ctx* c_, int id) : c(c_), b(nullptr) {
+        if (!c->timing || c->spans->size() >= MAX_SPANS) return;
+        cudaEvent_t a;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { (void)cudaGetLastError(); b = nullptr; return; }
+        cudaEventRecord(a, c->stream);
+        c->spans->push_back({id, a, b});
+    }
+    ~SpanGuard() { if (b) cudaEventRecord(b, c->stream); }
+};
+
+static void resolve_spans(fvnl_ctx* c) {
+    if (!c->spans) return;
+    for (auto& s : *c->spans) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(s.b) == cudaSuccess && cudaEventElapsedTime(&ms, s.a, s.b) == cudaSuccess) {
+            c->span_ms[s.id] += ms;
+            c->span_n[s.id] += 1;
+        }
+        cudaEventDestroy(s.a);
+        cudaEventDestroy(s.b);
+    }
+    (void)cudaGetLastError();
+    c->spans->clear();
+}
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 static const size_t CLOCK_BYTES = 256;
@@ -146,6 +184,8 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
     fvnl_ctx* c = new (std::nothrow) fvnl_ctx();
     if (!c) return FVNL_EALLOC;
     std::memset(c, 0, sizeof(*c));
+    c->spans = new (std::nothrow) std::vector<fvnl_ctx::Span>();
+    if (!c->spans) { delete c; return FVNL_EALLOC; }
     if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return FVNL_ECUDA; }
     c->g.nx = nx; c->g.ny = ny; c->g.dx = dx; c->g.dy = dy;
     c->g.c0 = m->c0; c->g.beta = m->beta; c->g.delta = m->delta;
@@ -191,6 +231,8 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
 extern "C" void fvnl_destroy(fvnl_ctx* c) {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
+    resolve_spans(c);
+    delete c->spans;
     for (int k = 0; k < 3; ++k)
         if (c->star[k]) cudaFree(c->star[k]);
     if (c->host_clk) cudaFreeHost(c->host_clk);
@@ -219,6 +261,10 @@ extern "C" int fvnl_set_option(fvnl_ctx* c, int option, int value) {
     if (option == FVNL_OPT_KERNEL) {
         if (value != FVNL_KERNEL_DEFAULT && value != FVNL_KERNEL_UNFUSED) return FVNL_EARG;
         c->kernel = value;
+        return FVNL_OK;
+    }
+    if (option == FVNL_OPT_KERNEL_TIMING) {
+        c->timing = value != 0;
         return FVNL_OK;
     }
     return FVNL_EARG;
@@ -296,9 +342,12 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
         double** b = c->buf[c->cur ^ 1];
         {
             const dim3 grdx((g.nx + 255) / 256, g.ny + 4);
-            k_xsweep_unfused<<<grdx, blk, 0, st>>>(g, c->clk, a[0], a[1], a[2], c->star[0], c->star[1], c->star[2]);
-            k_ysweep_unfused<<<grd, blk, 0, st>>>(g, c->clk, c->star[0], c->star[1], c->star[2], b[0], b[1], b[2]);
-            k_source_unfused<<<grd, blk, 0, st>>>(g, c->clk, b[0], b[1], b[2], a[0], a[1], a[2]);
+            { SpanGuard sp(c, FVNL_TIMED_XSWEEP);
+              k_xsweep_unfused<<<grdx, blk, 0, st>>>(g, c->clk, a[0], a[1], a[2], c->star[0], c->star[1], c->star[2]); }
+            { SpanGuard sp(c, FVNL_TIMED_YSWEEP);
+              k_ysweep_unfused<<<grd, blk, 0, st>>>(g, c->clk, c->star[0], c->star[1], c->star[2], b[0], b[1], b[2]); }
+            { SpanGuard sp(c, FVNL_TIMED_SOURCE);
+              k_source_unfused<<<grd, blk, 0, st>>>(g, c->clk, b[0], b[1], b[2], a[0], a[1], a[2]); }
             c->launches += 3;
             // result is back in `a`: cur unchanged
         }
@@ -331,6 +380,17 @@ extern "C" int fvnl_get_info(fvnl_ctx* c, double* t_s, double* last_dt_s, double
     if (last_cfl) *last_cfl = c->snap.last_cfl;
     if (last_M) *last_M = c->snap.Mprev;
     if (steps) *steps = (long)c->snap.steps;
+    return FVNL_OK;
+}
+
+extern "C" int fvnl_get_kernel_time(fvnl_ctx* c, int which, double* total_ms, long* launches) {
+    if (!c || which < 0 || which >= FVNL_TIMED_KINDS) return FVNL_EARG;
+    CK(cudaStreamSynchronize(c->stream));
+    resolve_spans(c);
+    if (total_ms) *total_ms = c->span_ms[which];
+    if (launches) *launches = c->span_n[which];
+    c->span_ms[which] = 0.0;
+    c->span_n[which] = 0;
     return FVNL_OK;
 }
 
