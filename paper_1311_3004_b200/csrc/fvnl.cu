@@ -333,7 +333,7 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
     }
     k_clock_begin<<<1, 1, 0, st>>>(g, c->clk, value, mode);
     c->launches += 1;
-    if (c->kernel == FVNL_KERNEL_UNFUSED) {
+    {   // TODO(fused): until fvnl_fused.cuh lands both kernel options run the three-pass form
         const int rc = ensure_star(c);
         if (rc) return rc;
     }
