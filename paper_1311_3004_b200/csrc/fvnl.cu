@@ -9,7 +9,7 @@
 #include <vector>
 
 #include "../../include/fvnl.h"
-#include "fvnl_unfused.cuh"
+#include "fvnl_fused.cuh"
 
 using namespace fvnl;
 
@@ -117,6 +117,7 @@ struct fvnl_ctx {
     bool have_state;
     bool need_prepass;
     int kernel;                 // FVNL_KERNEL_*
+    int rows_per_block;         // fused kernel: rows per chunk (0 = automatic)
     long launches;
     // opt-in per-kernel timing (FVNL_OPT_KERNEL_TIMING): event pairs around the sweep kernels, resolved on demand
     bool timing;
@@ -263,6 +264,11 @@ extern "C" int fvnl_set_option(fvnl_ctx* c, int option, int value) {
         c->kernel = value;
         return FVNL_OK;
     }
+    if (option == FVNL_OPT_ROWS_PER_BLOCK) {
+        if (value < 0) return FVNL_EARG;
+        c->rows_per_block = value;
+        return FVNL_OK;
+    }
     if (option == FVNL_OPT_KERNEL_TIMING) {
         c->timing = value != 0;
         return FVNL_OK;
@@ -308,6 +314,31 @@ static int ensure_star(fvnl_ctx* c) {
     return FVNL_OK;
 }
 
+// Fused step: strips of FUSED_BX columns (FUSED_BX - 6 produce output) x chunks of `rows` rows.
+static const int FUSED_BX = 256;
+
+static int fused_rows(const fvnl_ctx* c, int strips) {
+    if (c->rows_per_block > 0) return c->rows_per_block < c->g.ny ? c->rows_per_block : c->g.ny;
+    // enough blocks to fill the machine several times over, chunks not shorter than 64 rows (6 halo rows each)
+    const int ny = c->g.ny;
+    const int want_blocks = 148 * 2 * 8;
+    int chunks = (want_blocks + strips - 1) / strips;
+    int rows = (ny + chunks - 1) / chunks;
+    if (rows < 64) rows = 64;
+    if (rows > 512) rows = 512;
+    if (rows > ny) rows = ny;
+    return rows;
+}
+
+static void launch_fused(fvnl_ctx* c, double** a, double** b) {
+    const Grid& g = c->g;
+    const int strips = (g.nx + (FUSED_BX - 6) - 1) / (FUSED_BX - 6);
+    const int rows = fused_rows(c, strips);
+    const dim3 grd(strips, (g.ny + rows - 1) / rows);
+    SpanGuard sp(c, FVNL_TIMED_STEP);
+    k_step_fused<FUSED_BX><<<grd, FUSED_BX, 0, c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
+}
+
 static int read_clock(fvnl_ctx* c) {
     CK(cudaMemcpyAsync(c->host_clk, c->clk, sizeof(Clock), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
@@ -333,14 +364,18 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
     }
     k_clock_begin<<<1, 1, 0, st>>>(g, c->clk, value, mode);
     c->launches += 1;
-    {   // TODO(fused): until fvnl_fused.cuh lands both kernel options run the three-pass form
+    if (c->kernel == FVNL_KERNEL_UNFUSED) {
         const int rc = ensure_star(c);
         if (rc) return rc;
     }
     for (long n = 0; n < nsteps; ++n) {
         double** a = c->buf[c->cur];
         double** b = c->buf[c->cur ^ 1];
-        {
+        if (c->kernel == FVNL_KERNEL_DEFAULT) {
+            launch_fused(c, a, b);
+            c->launches += 1;
+            c->cur ^= 1;
+        } else {
             const dim3 grdx((g.nx + 255) / 256, g.ny + 4);
             { SpanGuard sp(c, FVNL_TIMED_XSWEEP);
               k_xsweep_unfused<<<grdx, blk, 0, st>>>(g, c->clk, a[0], a[1], a[2], c->star[0], c->star[1], c->star[2]); }
