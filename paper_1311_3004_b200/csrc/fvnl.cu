@@ -315,7 +315,7 @@ static int ensure_star(fvnl_ctx* c) {
 }
 
 // Fused step: strips of FUSED_BX columns (FUSED_BX - 6 produce output) x chunks of `rows` rows.
-static const int FUSED_BX = 256;
+static const int FUSED_BX = 256, FUSED_MINB = 2;
 
 static int fused_rows(const fvnl_ctx* c, int strips) {
     if (c->rows_per_block > 0) return c->rows_per_block < c->g.ny ? c->rows_per_block : c->g.ny;
@@ -335,8 +335,15 @@ static void launch_fused(fvnl_ctx* c, double** a, double** b) {
     const int strips = (g.nx + (FUSED_BX - 6) - 1) / (FUSED_BX - 6);
     const int rows = fused_rows(c, strips);
     const dim3 grd(strips, (g.ny + rows - 1) / rows);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_step_fused<FUSED_BX, FUSED_MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             fused_smem_bytes<FUSED_BX>());
+        attr_set = true;
+    }
     SpanGuard sp(c, FVNL_TIMED_STEP);
-    k_step_fused<FUSED_BX><<<grd, FUSED_BX, 0, c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
+    k_step_fused<FUSED_BX, FUSED_MINB><<<grd, FUSED_BX, fused_smem_bytes<FUSED_BX>(), c->stream>>>(
+        g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
 }
 
 static int read_clock(fvnl_ctx* c) {

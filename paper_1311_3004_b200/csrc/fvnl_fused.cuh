@@ -12,6 +12,11 @@
 // waves, fluctuations and the intermediate states Q*, Q** never touch HBM (PAPER.md:159-198 quantities live in
 // registers; the x-neighbour exchange goes through 17 doubles of shared memory per column).
 //
+// The path is bound by instruction issue and the FP64 pipe, not by HBM, so the code below is
+// arranged for instruction count: the tick loop is unrolled by two with the roles of the two register sets
+// exchanged (no register moves for the rolling window), the upwind neighbour in x is chosen by address, the upwind
+// neighbour in y by keeping one "pending" limiter input per wave, shared memory is laid out for 128-bit accesses.
+//
 // Ghost cells (readings A9, A10, A14 of DESIGN.md) are evaluated on load: the x rule maps the thread's column once,
 // the y rule maps the row of each tick; the one-deep ghosts of Q** that the source step needs are derived from the
 // neighbouring interior Q** at the edge columns / rows.
@@ -60,183 +65,351 @@ __device__ __forceinline__ RowMap map_row(const Grid& g, int r) {
     return m;
 }
 
-// Analytic override of a loaded ghost value (same precedence as load_ext: x rule first, then y rule).
-__device__ __noinline__ void apply_sources(const Grid& g, const ColMap& cm, const RowMap& rm, int i, int r, double t,
-                                           Q3& c) {
-    if (cm.xsrc >= 0) {
-        Q3 s;
-        if (source_cell(g.side[cm.xsrc], cm.xsrc, g.c0, (r + 0.5) * g.dy, (i + 0.5) * g.dx, t, s)) { c = s; return; }
+// Analytic override of a loaded ghost value (same precedence as load_ext: x rule first, then y rule).  Rare path:
+// everything by value so that nothing of the caller is forced into local memory.
+__device__ __noinline__ double3 apply_sources(Grid g, int xsrc, int ysrc, int col, bool neg2, int i, int r, double t,
+                                              double c1, double c2, double c3) {
+    Q3 s;
+    if (xsrc >= 0 && source_cell(g.side[xsrc], xsrc, g.c0, (r + 0.5) * g.dy, (i + 0.5) * g.dx, t, s))
+        return make_double3(s.q1, s.q2, s.q3);
+    if (ysrc >= 0) {
+        const double x = (col + 0.5) * g.dx;                    // the (x-mapped) column the y rule is applied on
+        if (source_cell(g.side[ysrc], ysrc, g.c0, x, x, t, s)) return make_double3(s.q1, neg2 ? -s.q2 : s.q2, s.q3);
     }
-    if (rm.ysrc >= 0) {
+    return make_double3(c1, c2, c3);
+}
+
+// z = (q2/q1, q3/q1) of the one-deep ghost of an intermediate state, from the z of the interior cell next to the
+// edge (source step, reading A9): EXTRAP copies, REFLECT negates the normal velocity, SOURCE is analytic inside the
+// aperture and EXTRAP outside.  (PERIODIC edges never come here.)
+__device__ __noinline__ double2 ghost_z(Grid g, int sd, double along, double xc, double t, double z2, double z3) {
+    const int kind = g.side[sd].kind;
+    if (kind == BC_REFLECT) return sd < 2 ? make_double2(-z2, z3) : make_double2(z2, -z3);
+    if (kind == BC_SOURCE) {
         Q3 s;
-        const double x = (cm.col + 0.5) * g.dx;                 // the (x-mapped) column the y rule is applied on
-        if (source_cell(g.side[rm.ysrc], rm.ysrc, g.c0, x, x, t, s)) {
-            if (cm.neg2) s.q2 = -s.q2;
-            c = s;
+        if (source_cell(g.side[sd], sd, g.c0, along, xc, t, s)) {
+            const double rc = rcp_o1(s.q1);
+            return make_double2(s.q2 * rc, s.q3 * rc);
         }
     }
+    return make_double2(z2, z3);
 }
 
-// z = (q2/q1, q3/q1) of the one-deep ghost of an intermediate state (source step, reading A9).
-__device__ __noinline__ void ghost_z(const Grid& g, int sd, const Q3& inner, double along, double xc, double t,
-                                     double& z2, double& z3) {
-    const Q3 c = ghost_of(g, sd, inner, along, xc, t);
-    const double rc = rcp_o1(c.q1);
-    z2 = c.q2 * rc;
-    z3 = c.q3 * rc;
-}
+// ---- per-interface arithmetic, arranged for instruction count --------------------------------------------------
+// (same formulas as fvnl_math.cuh -- PAPER.md:218-245, 169-198 -- with the pieces the fused kernel shares split out)
 
-struct WaveLite {                 // what a neighbouring interface contributes to the limiter
-    double al1, s1, r31, al2, s2, r32, al3;
+struct Cx {                       // a cell in sweep form: q2 normal, q3 transverse momentum; half primitive velocities
+    double q1, q2, q3, hz2, hz3;
 };
 
-// The step kernel.  grid = (strips, chunks); block = BX threads.  rows: rows of output per chunk.
+struct Wv {                       // Riemann solution at an interface: W1 = al1 (1,s1,r31), W2 = al2 (1,s2,r32), W3 = (0,0,al3)
+    double al1, s1, r31, al2, s2, r32, al3, v;      // v = s3
+};
+
+__device__ __forceinline__ Cx cell_of(double q1, double q2, double q3, int& min_q1hi) {
+    min_q1hi = min(min_q1hi, hi_word(q1));                      // q1 <= 0 shows as a non-positive high word
+    Cx c;
+    c.q1 = q1; c.q2 = q2; c.q3 = q3;
+    const double hr = 0.5 * rcp_o1(q1);
+    c.hz2 = q2 * hr;
+    c.hz3 = q3 * hr;
+    return c;
+}
+
+// b2 = 2(beta-1), omb2 = 1 - b2.  min_dhi tracks the sign of the square-root argument of (32),(33).
+__device__ __forceinline__ Wv riemann2(const Cx& L, const Cx& R, double b2, double omb2, int& min_dhi) {
+    Wv w;
+    const double D1 = R.q1 - L.q1, D2 = R.q2 - L.q2, D3 = R.q3 - L.q3;
+    const double Zb1 = fma(0.5, D1, L.q1);
+    const double Zb2 = L.hz2 + R.hz2;
+    const double Zb3 = L.hz3 + R.hz3;
+    const double Phi = fma(b2, Zb1, omb2);
+    const double u = rcp_o1(Zb1);
+    const double v = Zb2 * u;                                    // (34)
+    const double wv = Zb3 * u;
+    const double tt = fma(-2.0, Zb2, v);
+    const double disc = fma(v, tt, Phi);                         // (32),(33)
+    min_dhi = min(min_dhi, hi_word(disc));
+    const double ra = rsqrt_o1(disc);
+    w.s1 = fma(disc, ra, v);                                     // v + a
+    w.s2 = fma(-disc, ra, v);                                    // v - a
+    w.v = v;
+    const double hra = 0.5 * ra;
+    w.al1 = fma(-w.s2, D1, D2) * hra;
+    w.al2 = D1 - w.al1;
+    const double wra = wv * ra;
+    w.r31 = wra * fma(-2.0, Zb2, w.s1);                          //  w (s1 - 2 Zb2)/a
+    w.r32 = wra * fma(2.0, Zb2, -w.s2);                          // -w (s2 - 2 Zb2)/a
+    w.al3 = fma(-w.al2, w.r32, fma(-w.al1, w.r31, D3));
+    return w;
+}
+
+// 1/(r.r) of waves 1 and 2 (denominator of theta).
+__device__ __forceinline__ double rnorm(double s, double r3) { return rcp_o1(fma(s, s, fma(r3, r3, 1.0))); }
+
+// r_K . r_k of two neighbouring interfaces (symmetric), waves 1 / 2.
+__device__ __forceinline__ double rdot(double sK, double r3K, double s, double r3) { return fma(sK, s, fma(r3K, r3, 1.0)); }
+
+struct Fl {                       // left-going (m) and right-going (p) parts of an interface's contribution to (27)
+    double m1, m2, m3, p1, p2, p3;
+};
+
+// k: the interface; b_p = alpha_K^p (r_K.r_k)/(r_k.r_k) of the upwind interface K (b3 = alpha_K^3).  (28)-(30).
+__device__ __forceinline__ Fl flux2(const Wv& k, double b1, double b2, double b3, double lam) {
+    const double a1 = fabs(k.s1), a2 = fabs(k.s2), a3 = fabs(k.v);
+    const double f1 = a1 * fma(-lam, a1, 1.0) * mc_half(k.al1, b1);
+    const double f2 = a2 * fma(-lam, a2, 1.0) * mc_half(k.al2, b2);
+    const double f3 = a3 * fma(-lam, a3, 1.0) * mc_half(k.al3, b3);
+    const double g1m = fma(neg_part(k.s1), k.al1, f1), g1p = fma(k.s1, k.al1, -g1m);
+    const double g2m = fma(neg_part(k.s2), k.al2, f2), g2p = fma(k.s2, k.al2, -g2m);
+    const double g3m = fma(neg_part(k.v), k.al3, f3), g3p = fma(k.v, k.al3, -g3m);
+    Fl F;
+    F.m1 = g1m + g2m;
+    F.m2 = fma(g1m, k.s1, g2m * k.s2);
+    F.m3 = fma(g1m, k.r31, fma(g2m, k.r32, g3m));
+    F.p1 = g1p + g2p;
+    F.p2 = fma(g1p, k.s1, g2p * k.s2);
+    F.p3 = fma(g1p, k.r31, fma(g2p, k.r32, g3p));
+    return F;
+}
+
+// Rolling y-state of one interface (the newest one): its cell on the high side, waves, 1/(r.r), and the limiter
+// inputs it would take from the interface below it (used if that one is its upwind side).
+struct YSet {
+    Cx c;
+    Wv w;
+    double rn1, rn2;
+    double pb1, pb2, pb3;
+};
+
+// Shared-memory layout: one record per column, strides chosen as odd multiples of 16 B so that 128-bit accesses
+// of consecutive columns are bank-conflict free; one pad record on each side so that tid-1 / tid+1 never clamp.
+constexpr int SM_CELL = 48, SM_WAVE = 80, SM_GM = 48, SM_Z = 16;
+
+__device__ __forceinline__ void sts2(char* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
+__device__ __forceinline__ double2 lds2(const char* p) { return *reinterpret_cast<const double2*>(p); }
+__device__ __forceinline__ void sts1(char* p, double a) { *reinterpret_cast<double*>(p) = a; }
+__device__ __forceinline__ double lds1(const char* p) { return *reinterpret_cast<const double*>(p); }
+
+// Block-invariant quantities of a step.
+struct StepK {
+    double t, lamx, lamy, kapx, kapy, k2;    // k2 = -2 (kapx + kapy)
+    double b2, omb2;                         // 2 (beta - 1), 1 - b2
+    int j0, j1;                              // rows of output of this chunk: [j0, j1)
+    bool px, py, any_src, any_refl;
+};
+
+// Per-thread constants and running reductions.
+struct ThreadK {
+    ColMap cm;
+    int i;                                   // column on the ghost-extended mesh
+    bool fixW, fixE, out_col;
+    char *p_cell, *p_wave, *p_gm, *p_z;      // this column's shared-memory records
+    // running reductions (masked by validity at the end)
+    double smx, smy;
+    int mqx, mdx, mqy, mdy, mxo;             // min high words of q1 / disc in x and y; max |high word| of the output
+};
+
+// Carried between ticks besides the two YSets.
+struct Carry {
+    double n1, n2, n3;                       // prefetched row r+1 of Q^n
+    double gp1, gp2, gp3;                    // right-going part of the y-interface below the newest one, y-form
+    double c1, c2, c3, zC2, zC3;             // Q**(r-3) and its z
+    double zS2, zS3;                         // z of Q**(r-4)
+};
+
+// One tick.  A: the set of the newest y-interface so far, r-3/2 (its cell = Q*(r-1)); N: on entry its cell still
+// holds Q*(r-2) (from two ticks ago), on exit N is the set of interface r-1/2 (cell Q*(r)).
 template <int BX>
-__global__ void __launch_bounds__(BX) k_step_fused(Grid g, Clock* clk, const double* __restrict__ q1,
-                                                   const double* __restrict__ q2, const double* __restrict__ q3,
-                                                   double* __restrict__ o1, double* __restrict__ o2,
-                                                   double* __restrict__ o3, int rows) {
-    __shared__ double s_cell[5][BX];      // q1 q2 q3 hz2 hz3 of the cell of this column          (tick r)
-    __shared__ double s_wave[7][BX];      // al1 s1 r31 al2 s2 r32 al3 of the interface i-1/2      (tick r)
-    __shared__ double s_gm[3][BX];        // left-going part of the interface i-1/2                (tick r)
-    __shared__ double s_z[2][BX];         // q2/q1, q3/q1 of Q**                                   (row r-2)
-
-    const int tid = threadIdx.x;
-    const int i = (int)blockIdx.x * (BX - 6) - 3 + tid;            // column on the ghost-extended mesh
-    const int j0 = (int)blockIdx.y * rows;
-    const int j1 = min(j0 + rows, g.ny);
-    const double t = clk->t, lamx = clk->lamx, lamy = clk->lamy, kapx = clk->kapx, kapy = clk->kapy;
-    const double b2 = 2.0 * (g.beta - 1.0);
-    const bool px = g.side[SIDE_XLO].kind == BC_PERIODIC, py = g.side[SIDE_YLO].kind == BC_PERIODIC;
-    const bool any_src = g.side[0].kind == BC_SOURCE || g.side[1].kind == BC_SOURCE || g.side[2].kind == BC_SOURCE ||
-                         g.side[3].kind == BC_SOURCE;
-
-    const ColMap cm = map_column(g, i);
-    const int tl = tid > 0 ? tid - 1 : 0, tr = tid < BX - 1 ? tid + 1 : BX - 1;
-    // which results of this thread are real
-    const bool x_if_m = tid >= 1 && i >= 0 && i <= g.nx;           // interface i-1/2 enters M (touches an interior cell)
-    const bool x_if_f = tid >= 1 && i >= -1 && i <= g.nx + 1;      // interface i-1/2 is one the scheme solves
-    const bool y_col = tid >= 2 && tid <= BX - 3 && i >= 0 && i < g.nx;   // Q* of this column is valid and interior
-    const bool out_col = tid >= 3 && tid <= BX - 4 && i >= 0 && i < g.nx;
-    const bool fixW = !px && i == 0, fixE = !px && i == g.nx - 1;
-
-    int flags = 0;
-    double smx = 0.0, smy = 0.0;
-
-    // rolling state (all in y-form where noted: components 2 and 3 switched)
-    CellX cyA = {1.0, 0.0, 0.0, 0.0, 0.0};                        // y-cell of Q*(r-1)
-    double sB1 = 1.0, sB2 = 0.0, sB3 = 0.0;                        // Q*(r-2), y-form
-    Waves wA = {0, 1, 0, 0, -1, 0, 0, 0}, wB = wA;                 // Wy(r-3/2), Wy(r-5/2)
-    double gB1 = 0.0, gB2 = 0.0, gB3 = 0.0;                        // right-going part of the y-interface r-5/2
-    double c1 = 1.0, c2 = 0.0, c3 = 0.0, zC2 = 0.0, zC3 = 0.0, lC2 = 0.0, lC3 = 0.0;   // Q**(r-3), its z and d2x z
-    double zS2 = 0.0, zS3 = 0.0;                                   // z of Q**(r-4)
-
-    // first row
-    int r = j0 - 3;
-    RowMap rm = map_row(g, r);
-    size_t idx = (size_t)rm.row * g.nx + cm.col;
-    Q3 nxt;
-    nxt.q1 = q1[idx]; nxt.q2 = q2[idx]; nxt.q3 = q3[idx];
-
-    for (; r < j1 + 3; ++r) {
-        // ---- this tick's cell; prefetch the next row --------------------------------------------------------
-        Q3 q = nxt;
-        if (cm.neg2) q.q2 = -q.q2;
-        if (rm.neg3) q.q3 = -q.q3;
-        if (any_src && (cm.xsrc >= 0 || rm.ysrc >= 0)) apply_sources(g, cm, rm, i, r, t, q);
-        const RowMap rm_next = map_row(g, r + 1);
-        idx = (size_t)rm_next.row * g.nx + cm.col;
-        nxt.q1 = q1[idx]; nxt.q2 = q2[idx]; nxt.q3 = q3[idx];
-        const bool row_in = r >= 0 && r < g.ny;
-
-        // ---- x-sweep of row r (27)-(30) ---------------------------------------------------------------------
-        int fx = 0;
-        const CellX cx = make_cell(q.q1, q.q2, q.q3, fx);
-        s_cell[0][tid] = cx.q1; s_cell[1][tid] = cx.q2; s_cell[2][tid] = cx.q3; s_cell[3][tid] = cx.hz2; s_cell[4][tid] = cx.hz3;
-        __syncthreads();
-        CellX L;
-        L.q1 = s_cell[0][tl]; L.q2 = s_cell[1][tl]; L.q3 = s_cell[2][tl]; L.hz2 = s_cell[3][tl]; L.hz3 = s_cell[4][tl];
-        const Waves w = riemann_x(L, cx, b2, fx);
-        s_wave[0][tid] = w.al1; s_wave[1][tid] = w.s1; s_wave[2][tid] = w.r31; s_wave[3][tid] = w.al2;
-        s_wave[4][tid] = w.s2; s_wave[5][tid] = w.r32; s_wave[6][tid] = w.al3;
-        __syncthreads();
-        Flux3 F;
-        {
-            const int u1 = w.s1 > 0.0 ? tl : tr, u2 = w.s2 > 0.0 ? tl : tr, u3 = w.s3 > 0.0 ? tl : tr;
-            F = interface_flux(w, s_wave[0][u1], s_wave[1][u1], s_wave[2][u1], s_wave[3][u2], s_wave[4][u2],
-                               s_wave[5][u2], s_wave[6][u3], lamx);
-        }
-        s_gm[0][tid] = F.m1; s_gm[1][tid] = F.m2; s_gm[2][tid] = F.m3;
-        if (row_in) {
-            if (x_if_m) smx = fmax(smx, max_speed(w));
-            if (x_if_f) flags |= fx;
-        }
-        __syncthreads();
-        Q3 st;                                                    // Q*(i, r)
-        st.q1 = fma(-lamx, F.p1 + s_gm[0][tr], q.q1);
-        st.q2 = fma(-lamx, F.p2 + s_gm[1][tr], q.q2);
-        st.q3 = fma(-lamx, F.p3 + s_gm[2][tr], q.q3);
-        if (row_in && y_col && (not_finite(st.q1) || not_finite(st.q2) || not_finite(st.q3))) flags |= F_ENAN;
-
-        // ---- y-sweep: interface r-1/2, flux of interface r-3/2, Q**(r-2) -------------------------------------
-        int fy = 0;
-        const CellX cyN = make_cell(st.q1, st.q3, st.q2, fy);
-        const Waves wN = riemann_x(cyA, cyN, b2, fy);
-        Flux3 G;
-        {
-            const bool u1 = wA.s1 > 0.0, u2 = wA.s2 > 0.0, u3 = wA.s3 > 0.0;
-            G = interface_flux(wA, u1 ? wB.al1 : wN.al1, u1 ? wB.s1 : wN.s1, u1 ? wB.r31 : wN.r31,
-                               u2 ? wB.al2 : wN.al2, u2 ? wB.s2 : wN.s2, u2 ? wB.r32 : wN.r32,
-                               u3 ? wB.al3 : wN.al3, lamy);
-        }
-        Q3 n;                                                     // Q**(i, r-2), physical component order
-        n.q1 = fma(-lamy, gB1 + G.m1, sB1);
-        n.q3 = fma(-lamy, gB2 + G.m2, sB2);
-        n.q2 = fma(-lamy, gB3 + G.m3, sB3);
-        if (y_col && r >= j0 - 2 && r >= -1 && r <= g.ny + 1) {   // interface r-1/2 is one the scheme solves
-            flags |= fy;
-            if (r >= 0 && r <= g.ny) smy = fmax(smy, max_speed(wN));
-        }
-        if (y_col && r >= j0 + 1 && r - 2 >= 0 && r - 2 < g.ny &&
-            (not_finite(n.q1) || not_finite(n.q2) || not_finite(n.q3))) flags |= F_ENAN;
-        gB1 = G.p1; gB2 = G.p2; gB3 = G.p3;
-        wB = wA; wA = wN;
-        sB1 = cyA.q1; sB2 = cyA.q2; sB3 = cyA.q3;
-        cyA = cyN;
-
-        // ---- source step (26): d2x z of row r-2 now, output row R = r-3 ---------------------------------------
-        const double rn = rcp_o1(n.q1);
-        const double zN2 = n.q2 * rn, zN3 = n.q3 * rn;
-        s_z[0][tid] = zN2; s_z[1][tid] = zN3;
-        __syncthreads();
-        double zW2 = s_z[0][tl], zW3 = s_z[1][tl], zE2 = s_z[0][tr], zE3 = s_z[1][tr];
-        if (fixW) ghost_z(g, SIDE_XLO, n, (r - 2 + 0.5) * g.dy, -0.5 * g.dx, t, zW2, zW3);
-        if (fixE) ghost_z(g, SIDE_XHI, n, (r - 2 + 0.5) * g.dy, (g.nx + 0.5) * g.dx, t, zE2, zE3);
-        const double lN2 = (zE2 + zW2) - 2.0 * zN2, lN3 = (zE3 + zW3) - 2.0 * zN3;
-        const int R = r - 3;
-        if (R >= j0) {                                            // R < j1 by the loop bound
-            double a2 = zS2, a3 = zS3, b2n = zN2, b3n = zN3;
-            if (!py) {
-                Q3 c; c.q1 = c1; c.q2 = c2; c.q3 = c3;
-                const double x = (i + 0.5) * g.dx;
-                if (R == 0) ghost_z(g, SIDE_YLO, c, x, x, t, a2, a3);
-                if (R == g.ny - 1) ghost_z(g, SIDE_YHI, c, x, x, t, b2n, b3n);
-            }
-            const double ly2 = (b2n + a2) - 2.0 * zC2, ly3 = (b3n + a3) - 2.0 * zC3;
-            if (out_col) {
-                const size_t o = (size_t)R * g.nx + i;
-                o1[o] = c1;
-                o2[o] = fma(kapy, ly2, fma(kapx, lC2, c2));
-                o3[o] = fma(kapy, ly3, fma(kapx, lC3, c3));
-            }
-        }
-        zS2 = zC2; zS3 = zC3;
-        c1 = n.q1; c2 = n.q2; c3 = n.q3; zC2 = zN2; zC3 = zN3; lC2 = lN2; lC3 = lN3;
-        rm = rm_next;
+__device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th, Carry& cy, const YSet& A, YSet& N, int r,
+                                     const RowMap rm, const RowMap rm_next, const double* __restrict__ q1,
+                                     const double* __restrict__ q2, const double* __restrict__ q3,
+                                     double* __restrict__ o1, double* __restrict__ o2, double* __restrict__ o3) {
+    // ---- this tick's cell of Q^n; prefetch the next row ------------------------------------------------------
+    double a1 = cy.n1, a2 = cy.n2, a3 = cy.n3;
+    if (k.any_refl) {
+        if (th.cm.neg2) a2 = -a2;
+        if (rm.neg3) a3 = -a3;
     }
-    block_max_to(&clk->sx_bits, smx);
+    if (k.any_src && (th.cm.xsrc >= 0 || rm.ysrc >= 0)) {
+        const double3 s = apply_sources(g, th.cm.xsrc, rm.ysrc, th.cm.col, th.cm.neg2, th.i, r, k.t, a1, a2, a3);
+        a1 = s.x; a2 = s.y; a3 = s.z;
+    }
+    {
+        const size_t idx = (size_t)rm_next.row * g.nx + th.cm.col;
+        cy.n1 = q1[idx]; cy.n2 = q2[idx]; cy.n3 = q3[idx];
+    }
+    const bool row_in = r >= 0 && r < g.ny;
+
+    // ---- x-sweep of row r: cells -> waves -> limited fluxes -> Q*(., r)      (27)-(30), PAPER.md:159-198 ------
+    int tq = 0x7fffffff, td = 0x7fffffff;
+    const Cx cx = cell_of(a1, a2, a3, tq);
+    sts2(th.p_cell, cx.q1, cx.q2); sts2(th.p_cell + 16, cx.q3, cx.hz2); sts1(th.p_cell + 32, cx.hz3);
+    __syncthreads();                                                          // B1: cells (and last tick's z) visible
+    Cx L;
+    {
+        const double2 u0 = lds2(th.p_cell - SM_CELL), u1 = lds2(th.p_cell - SM_CELL + 16);
+        L.q1 = u0.x; L.q2 = u0.y; L.q3 = u1.x; L.hz2 = u1.y; L.hz3 = lds1(th.p_cell - SM_CELL + 32);
+    }
+    // d2x z of row r-3 (its z was published at the end of the previous tick)
+    double2 zW = lds2(th.p_z - SM_Z), zE = lds2(th.p_z + SM_Z);
+    const Wv w = riemann2(L, cx, k.b2, k.omb2, td);
+    const double rn1 = rnorm(w.s1, w.r31), rn2 = rnorm(w.s2, w.r32);
+    sts2(th.p_wave, w.al1, w.s1); sts2(th.p_wave + 16, w.r31, w.al3); sts2(th.p_wave + 32, w.al2, w.s2);
+    sts1(th.p_wave + 48, w.r32);
+    if (row_in) {
+        th.mqx = min(th.mqx, tq); th.mdx = min(th.mdx, td);
+        th.smx = fmax(th.smx, fabs(hi_word(w.v) < 0 ? w.s2 : w.s1));          // max(|s1|,|s2|) = |v| + a
+    }
+    __syncthreads();                                                          // B2: waves visible
+    Fl F;
+    {
+        const char* u1 = th.p_wave + (hi_word(w.s1) < 0 ? SM_WAVE : -SM_WAVE);   // upwind interface
+        const char* u2 = th.p_wave + (hi_word(w.s2) < 0 ? SM_WAVE : -SM_WAVE);
+        const char* u3 = th.p_wave + (hi_word(w.v) < 0 ? SM_WAVE : -SM_WAVE);
+        const double2 k1 = lds2(u1), k2 = lds2(u2 + 32);
+        const double k1r = lds1(u1 + 16), k2r = lds1(u2 + 48), k3 = lds1(u3 + 24);
+        const double b1 = k1.x * rdot(k1.y, k1r, w.s1, w.r31) * rn1;
+        const double b2 = k2.x * rdot(k2.y, k2r, w.s2, w.r32) * rn2;
+        F = flux2(w, b1, b2, k3, k.lamx);
+    }
+    sts2(th.p_gm, F.m1, F.m2); sts1(th.p_gm + 16, F.m3);
+    // source step, x part for row r-3 (independent of the barriers above; placed here to fill the wait)
+    if (th.fixW) zW = ghost_z(g, SIDE_XLO, (r - 3 + 0.5) * g.dy, -0.5 * g.dx, k.t, cy.zC2, cy.zC3);
+    if (th.fixE) zE = ghost_z(g, SIDE_XHI, (r - 3 + 0.5) * g.dy, (g.nx + 0.5) * g.dx, k.t, cy.zC2, cy.zC3);
+    const double H2 = fma(k.k2, cy.zC2, fma(k.kapx, zE.x + zW.x, cy.c2));
+    const double H3 = fma(k.k2, cy.zC3, fma(k.kapx, zE.y + zW.y, cy.c3));
+    __syncthreads();                                                          // B3: left-going parts visible
+    double s1, s2, s3;                                                        // Q*(i, r)
+    {
+        const double2 gm = lds2(th.p_gm + SM_GM);
+        const double gm3 = lds1(th.p_gm + SM_GM + 16);
+        s1 = fma(-k.lamx, F.p1 + gm.x, a1);
+        s2 = fma(-k.lamx, F.p2 + gm.y, a2);
+        s3 = fma(-k.lamx, F.p3 + gm3, a3);
+    }
+
+    // ---- y-sweep: interface r-1/2 (N), limited flux of interface r-3/2 (A), Q**(., r-2) ------------------------
+    const double b1o = N.c.q1, b2o = N.c.q2, b3o = N.c.q3;                    // Q*(r-2), y-form (before N is overwritten)
+    int tqy = 0x7fffffff, tdy = 0x7fffffff;
+    N.c = cell_of(s1, s3, s2, tqy);                                           // positions 2,3 switched
+    N.w = riemann2(A.c, N.c, k.b2, k.omb2, tdy);
+    N.rn1 = rnorm(N.w.s1, N.w.r31); N.rn2 = rnorm(N.w.s2, N.w.r32);
+    const double d1 = rdot(A.w.s1, A.w.r31, N.w.s1, N.w.r31), d2 = rdot(A.w.s2, A.w.r32, N.w.s2, N.w.r32);
+    N.pb1 = A.w.al1 * d1 * N.rn1; N.pb2 = A.w.al2 * d2 * N.rn2; N.pb3 = A.w.al3;      // if A is N's upwind side
+    const double hb1 = N.w.al1 * d1 * A.rn1, hb2 = N.w.al2 * d2 * A.rn2;              // if N is A's upwind side
+    const Fl G = flux2(A.w, hi_word(A.w.s1) < 0 ? hb1 : A.pb1, hi_word(A.w.s2) < 0 ? hb2 : A.pb2,
+                       hi_word(A.w.v) < 0 ? N.w.al3 : A.pb3, k.lamy);
+    const double n1 = fma(-k.lamy, cy.gp1 + G.m1, b1o);                       // Q**(i, r-2); physical order: n1, n2, n3
+    const double n3 = fma(-k.lamy, cy.gp2 + G.m2, b2o);
+    const double n2 = fma(-k.lamy, cy.gp3 + G.m3, b3o);
+    cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3;
+    if (r >= k.j0 - 2 && r >= -1 && r <= g.ny + 1) {                          // interface r-1/2 is one the scheme solves
+        th.mqy = min(th.mqy, tqy); th.mdy = min(th.mdy, tdy);
+        if (r >= 0 && r <= g.ny) th.smy = fmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
+    }
+
+    // ---- source step (26): publish z of row r-2, finish row R = r-3 ---------------------------------------------
+    const double rq = rcp_o1(n1);
+    const double zN2 = n2 * rq, zN3 = n3 * rq;
+    sts2(th.p_z, zN2, zN3);                                                   // read after B1 of the next tick
+    const int R = r - 3;
+    if (R >= k.j0) {                                                          // R < j1 by the loop bound
+        double y2 = zN2 + cy.zS2, y3 = zN3 + cy.zS3;
+        if (!k.py && (R == 0 || R == g.ny - 1)) {
+            const double x = (th.i + 0.5) * g.dx;
+            double2 lo = make_double2(cy.zS2, cy.zS3), hi = make_double2(zN2, zN3);
+            if (R == 0) lo = ghost_z(g, SIDE_YLO, x, x, k.t, cy.zC2, cy.zC3);
+            if (R == g.ny - 1) hi = ghost_z(g, SIDE_YHI, x, x, k.t, cy.zC2, cy.zC3);
+            y2 = hi.x + lo.x; y3 = hi.y + lo.y;
+        }
+        const double w2 = fma(k.kapy, y2, H2), w3 = fma(k.kapy, y3, H3);
+        if (th.out_col) {
+            const size_t o = (size_t)R * g.nx + th.i;
+            o1[o] = cy.c1; o2[o] = w2; o3[o] = w3;
+            th.mxo = max(th.mxo, max(hi_word(cy.c1) & 0x7fffffff, max(hi_word(w2) & 0x7fffffff, hi_word(w3) & 0x7fffffff)));
+        }
+    }
+    cy.zS2 = cy.zC2; cy.zS3 = cy.zC3;
+    cy.c1 = n1; cy.c2 = n2; cy.c3 = n3; cy.zC2 = zN2; cy.zC3 = zN3;
+}
+
+template <int BX>
+__host__ __device__ constexpr int fused_smem_bytes() { return (BX + 2) * (SM_CELL + SM_WAVE + SM_GM + SM_Z); }
+
+// The step kernel.  grid = (strips, chunks); block = BX threads; dynamic shared memory = fused_smem_bytes<BX>().
+// rows: rows of output per chunk.
+template <int BX, int MINB>
+__global__ void __launch_bounds__(BX, MINB) k_step_fused(Grid g, Clock* clk, const double* __restrict__ q1,
+                                                         const double* __restrict__ q2, const double* __restrict__ q3,
+                                                         double* __restrict__ o1, double* __restrict__ o2,
+                                                         double* __restrict__ o3, int rows) {
+    extern __shared__ __align__(16) char smem[];
+    const int tid = threadIdx.x;
+    for (int k = tid; k < fused_smem_bytes<BX>() / 8; k += BX) reinterpret_cast<double*>(smem)[k] = 0.0;
+
+    StepK k;
+    k.t = clk->t; k.lamx = clk->lamx; k.lamy = clk->lamy; k.kapx = clk->kapx; k.kapy = clk->kapy;
+    k.k2 = -2.0 * (k.kapx + k.kapy);
+    k.b2 = 2.0 * (g.beta - 1.0); k.omb2 = 1.0 - k.b2;
+    k.j0 = (int)blockIdx.y * rows; k.j1 = min(k.j0 + rows, g.ny);
+    k.px = g.side[SIDE_XLO].kind == BC_PERIODIC; k.py = g.side[SIDE_YLO].kind == BC_PERIODIC;
+    k.any_src = g.side[0].kind == BC_SOURCE || g.side[1].kind == BC_SOURCE || g.side[2].kind == BC_SOURCE ||
+                g.side[3].kind == BC_SOURCE;
+    k.any_refl = g.side[0].kind == BC_REFLECT || g.side[1].kind == BC_REFLECT || g.side[2].kind == BC_REFLECT ||
+                 g.side[3].kind == BC_REFLECT;
+
+    ThreadK th;
+    th.i = (int)blockIdx.x * (BX - 6) - 3 + tid;
+    th.cm = map_column(g, th.i);
+    th.fixW = !k.px && th.i == 0; th.fixE = !k.px && th.i == g.nx - 1;
+    th.out_col = tid >= 3 && tid <= BX - 4 && th.i >= 0 && th.i < g.nx;
+    th.p_cell = smem + (tid + 1) * SM_CELL;
+    th.p_wave = smem + (BX + 2) * SM_CELL + (tid + 1) * SM_WAVE;
+    th.p_gm = smem + (BX + 2) * (SM_CELL + SM_WAVE) + (tid + 1) * SM_GM;
+    th.p_z = smem + (BX + 2) * (SM_CELL + SM_WAVE + SM_GM) + (tid + 1) * SM_Z;
+    th.smx = 0.0; th.smy = 0.0;
+    th.mqx = th.mdx = th.mqy = th.mdy = 0x7fffffff; th.mxo = 0;
+
+    YSet Y0, Y1;
+    Y0.c = {1.0, 0.0, 0.0, 0.0, 0.0};
+    Y0.w = {0.0, 1.0, 0.0, 0.0, -1.0, 0.0, 0.0, 0.0};
+    Y0.rn1 = Y0.rn2 = 0.5; Y0.pb1 = Y0.pb2 = Y0.pb3 = 0.0;
+    Y1 = Y0;
+    Carry cy;
+    cy.gp1 = cy.gp2 = cy.gp3 = 0.0;
+    cy.c1 = 1.0; cy.c2 = cy.c3 = cy.zC2 = cy.zC3 = cy.zS2 = cy.zS3 = 0.0;
+
+    int r = k.j0 - 3;
+    const int rend = k.j1 + 3;
+    RowMap rm = map_row(g, r);
+    {
+        const size_t idx = (size_t)rm.row * g.nx + th.cm.col;
+        cy.n1 = q1[idx]; cy.n2 = q2[idx]; cy.n3 = q3[idx];
+    }
     __syncthreads();
-    block_max_to(&clk->sy_bits, smy);
+    while (true) {
+        RowMap rmn = map_row(g, r + 1);
+        tick<BX>(g, k, th, cy, Y0, Y1, r, rm, rmn, q1, q2, q3, o1, o2, o3);
+        if (++r >= rend) break;
+        rm = map_row(g, r + 1);
+        tick<BX>(g, k, th, cy, Y1, Y0, r, rmn, rm, q1, q2, q3, o1, o2, o3);
+        if (++r >= rend) break;
+    }
+
+    // ---- reductions: M of and the sticky flags, masked by which results of this thread are real ----
+    const int i = th.i;
+    const bool x_if_m = tid >= 1 && i >= 0 && i <= g.nx;            // x-interface i-1/2 touches an interior cell
+    const bool x_if_f = tid >= 1 && i >= -1 && i <= g.nx + 1;       // ... is one the scheme solves
+    const bool x_cell = i >= -2 && i <= g.nx + 1;
+    const bool y_col = tid >= 2 && tid <= BX - 3 && i >= 0 && i < g.nx;
+    int flags = 0;
+    if ((x_cell && th.mqx <= 0) || (y_col && th.mqy <= 0)) flags |= F_ENONPOS;
+    if ((x_if_f && th.mdx < 0) || (y_col && th.mdy < 0)) flags |= F_ENONREAL;
+    if (th.mxo >= 0x7ff00000) flags |= F_ENAN;
+    block_max_to(&clk->sx_bits, x_if_m ? th.smx : 0.0);
+    __syncthreads();
+    block_max_to(&clk->sy_bits, y_col ? th.smy : 0.0);
     block_flags_to(&clk->flags, flags);
 }
 
