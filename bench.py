@@ -205,6 +205,10 @@ def run_gpu(args):
         s.set_bc(side, kind, src)
     if args.kernel == "unfused":
         s.set_option(P.OPT_KERNEL, P.KERNEL_UNFUSED)
+    if args.variant:
+        s.set_option(P.OPT_VARIANT, args.variant)
+    if args.rows:
+        s.set_option(P.OPT_ROWS_PER_BLOCK, args.rows)
     q0 = w.init(device=dev)                    # seeded synthetic state, generated on the device (resident in HBM)
     s.set_state(*q0)
     del q0
@@ -298,7 +302,7 @@ def run_gpu(args):
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": w.name, "grid": [w.nx, w.ny], "cells": w.cells, "bc": [k for k, _ in w.bc],
-                   "nu_W": w.value, "kernel": args.kernel, "state_bytes": 24 * w.cells,
+                   "nu_W": w.value, "kernel": args.kernel, "variant": args.variant, "rows_per_block": args.rows, "state_bytes": 24 * w.cells,
                    "l2": "state larger than L2, no flush" if 24 * w.cells > 4 * 126e6 else "state near/below L2 size",
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "flags": int(flags),
                    "t_end_s": info["t"], "last_cfl": info["cfl"]},
@@ -320,6 +324,8 @@ def main():
     ap.add_argument("--workload", default="C5-16384")
     ap.add_argument("--kernel", default="fused", choices=["fused", "unfused"])
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--variant", type=int, default=0, help="launch variant of the fused kernel (tuning aid)")
+    ap.add_argument("--rows", type=int, default=0, help="rows per block of the fused kernel (0 = automatic)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")

@@ -137,8 +137,10 @@ int fvnl_get_info(fvnl_ctx* ctx, double* t_s, double* last_dt_s, double* last_cf
  * the three-pass form (x-sweep, y-sweep, source step as separate kernels through HBM; allocates one more
  * y-extended state with cudaMalloc on first use) -- a measured comparison point for "what fusion buys" and an
  * independently structured second implementation for cross-checks.  Same results up to rounding.
- * FVNL_OPT_ROWS_PER_BLOCK: rows one thread block of the fused kernel marches over (0 = automatic). */
-enum { FVNL_OPT_KERNEL = 0, FVNL_OPT_ROWS_PER_BLOCK = 1, FVNL_OPT_KERNEL_TIMING = 2 };
+ * FVNL_OPT_ROWS_PER_BLOCK: rows one thread block of the fused kernel marches over (0 = automatic).
+ * FVNL_OPT_VARIANT: launch variant of the fused kernel (block width / register budget; 0 = default; tuning aid,
+ * results are identical for every variant). */
+enum { FVNL_OPT_KERNEL = 0, FVNL_OPT_ROWS_PER_BLOCK = 1, FVNL_OPT_KERNEL_TIMING = 2, FVNL_OPT_VARIANT = 3 };
 enum { FVNL_KERNEL_DEFAULT = 0, FVNL_KERNEL_UNFUSED = 1 };
 int fvnl_set_option(fvnl_ctx* ctx, int option, int value);
 

@@ -118,6 +118,7 @@ struct fvnl_ctx {
     bool need_prepass;
     int kernel;                 // FVNL_KERNEL_*
     int rows_per_block;         // fused kernel: rows per chunk (0 = automatic)
+    int variant;                // fused kernel: launch variant
     long launches;
     // opt-in per-kernel timing (FVNL_OPT_KERNEL_TIMING): event pairs around the sweep kernels, resolved on demand
     bool timing;
@@ -128,6 +129,7 @@ struct fvnl_ctx {
 };
 
 static const size_t MAX_SPANS = 1 << 16;
+static const int N_FUSED_VARIANTS = 4;     // launch variants of the fused kernel (launch_fused)
 
 // Event pair around one kernel launch (timing on only).
 struct SpanGuard {
@@ -269,6 +271,11 @@ extern "C" int fvnl_set_option(fvnl_ctx* c, int option, int value) {
         c->rows_per_block = value;
         return FVNL_OK;
     }
+    if (option == FVNL_OPT_VARIANT) {
+        if (value < 0 || value >= N_FUSED_VARIANTS) return FVNL_EARG;
+        c->variant = value;
+        return FVNL_OK;
+    }
     if (option == FVNL_OPT_KERNEL_TIMING) {
         c->timing = value != 0;
         return FVNL_OK;
@@ -314,14 +321,16 @@ static int ensure_star(fvnl_ctx* c) {
     return FVNL_OK;
 }
 
-// Fused step: strips of FUSED_BX columns (FUSED_BX - 6 produce output) x chunks of `rows` rows.
-static const int FUSED_BX = 256, FUSED_MINB = 2;
+// Fused step: strips of BX columns (BX - 6 produce output) x chunks of `rows` rows.  Launch variants
+// (FVNL_OPT_VARIANT): block width and the register budget the compiler was given (blocks per SM).
+struct FusedVariant { int bx, minb; };
+static const FusedVariant FUSED_VARIANTS[] = {{128, 3}, {256, 2}, {128, 4}, {256, 1}};
 
 static int fused_rows(const fvnl_ctx* c, int strips) {
     if (c->rows_per_block > 0) return c->rows_per_block < c->g.ny ? c->rows_per_block : c->g.ny;
     // enough blocks to fill the machine several times over, chunks not shorter than 64 rows (6 halo rows each)
     const int ny = c->g.ny;
-    const int want_blocks = 148 * 2 * 8;
+    const int want_blocks = 148 * 4 * 6;
     int chunks = (want_blocks + strips - 1) / strips;
     int rows = (ny + chunks - 1) / chunks;
     if (rows < 64) rows = 64;
@@ -330,20 +339,28 @@ static int fused_rows(const fvnl_ctx* c, int strips) {
     return rows;
 }
 
-static void launch_fused(fvnl_ctx* c, double** a, double** b) {
+template <int BX, int MINB>
+static void launch_fused_t(fvnl_ctx* c, double** a, double** b) {
     const Grid& g = c->g;
-    const int strips = (g.nx + (FUSED_BX - 6) - 1) / (FUSED_BX - 6);
+    const int strips = (g.nx + (BX - 6) - 1) / (BX - 6);
     const int rows = fused_rows(c, strips);
     const dim3 grd(strips, (g.ny + rows - 1) / rows);
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(k_step_fused<FUSED_BX, FUSED_MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             fused_smem_bytes<FUSED_BX>());
+        cudaFuncSetAttribute(k_step_fused<BX, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, fused_smem_bytes<BX>());
         attr_set = true;
     }
     SpanGuard sp(c, FVNL_TIMED_STEP);
-    k_step_fused<FUSED_BX, FUSED_MINB><<<grd, FUSED_BX, fused_smem_bytes<FUSED_BX>(), c->stream>>>(
-        g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
+    k_step_fused<BX, MINB><<<grd, BX, fused_smem_bytes<BX>(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
+}
+
+static void launch_fused(fvnl_ctx* c, double** a, double** b) {
+    switch (c->variant) {
+        case 1: launch_fused_t<256, 2>(c, a, b); break;
+        case 2: launch_fused_t<128, 4>(c, a, b); break;
+        case 3: launch_fused_t<256, 1>(c, a, b); break;
+        default: launch_fused_t<128, 3>(c, a, b); break;
+    }
 }
 
 static int read_clock(fvnl_ctx* c) {

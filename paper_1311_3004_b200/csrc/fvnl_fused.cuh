@@ -150,6 +150,20 @@ __device__ __forceinline__ double rnorm(double s, double r3) { return rcp_o1(fma
 // r_K . r_k of two neighbouring interfaces (symmetric), waves 1 / 2.
 __device__ __forceinline__ double rdot(double sK, double r3K, double s, double r3) { return fma(sK, s, fma(r3K, r3, 1.0)); }
 
+// Compare-and-select min / max (no NaN fix-up code: a NaN anywhere ends in the output, which is checked).
+__device__ __forceinline__ double dmin(double a, double b) { return b < a ? b : a; }
+__device__ __forceinline__ double dmax(double a, double b) { return b > a ? b : a; }
+
+// Half of phi(b/a) a, MC limiter, as mc_half of fvnl_math.cuh.
+__device__ __forceinline__ double mc_half2(double a, double b) {
+    const double A = fabs(a);
+    const double B = xor_sign(b, a);
+    const double q = 0.25 * (A + B);
+    const double m = dmin(dmin(A, B), q);
+    const double r = hi_word(m) < 0 ? 0.0 : m;
+    return xor_sign(r, a);
+}
+
 struct Fl {                       // left-going (m) and right-going (p) parts of an interface's contribution to (27)
     double m1, m2, m3, p1, p2, p3;
 };
@@ -157,9 +171,9 @@ struct Fl {                       // left-going (m) and right-going (p) parts of
 // k: the interface; b_p = alpha_K^p (r_K.r_k)/(r_k.r_k) of the upwind interface K (b3 = alpha_K^3).  (28)-(30).
 __device__ __forceinline__ Fl flux2(const Wv& k, double b1, double b2, double b3, double lam) {
     const double a1 = fabs(k.s1), a2 = fabs(k.s2), a3 = fabs(k.v);
-    const double f1 = a1 * fma(-lam, a1, 1.0) * mc_half(k.al1, b1);
-    const double f2 = a2 * fma(-lam, a2, 1.0) * mc_half(k.al2, b2);
-    const double f3 = a3 * fma(-lam, a3, 1.0) * mc_half(k.al3, b3);
+    const double f1 = a1 * fma(-lam, a1, 1.0) * mc_half2(k.al1, b1);
+    const double f2 = a2 * fma(-lam, a2, 1.0) * mc_half2(k.al2, b2);
+    const double f3 = a3 * fma(-lam, a3, 1.0) * mc_half2(k.al3, b3);
     const double g1m = fma(neg_part(k.s1), k.al1, f1), g1p = fma(k.s1, k.al1, -g1m);
     const double g2m = fma(neg_part(k.s2), k.al2, f2), g2p = fma(k.s2, k.al2, -g2m);
     const double g3m = fma(neg_part(k.v), k.al3, f3), g3p = fma(k.v, k.al3, -g3m);
@@ -213,19 +227,24 @@ struct ThreadK {
 // Carried between ticks besides the two YSets.
 struct Carry {
     double n1, n2, n3;                       // prefetched row r+1 of Q^n
+    double s1, s2, s3;                       // Q*(., r-1), left by the previous tick for the y-sweep
     double gp1, gp2, gp3;                    // right-going part of the y-interface below the newest one, y-form
     double c1, c2, c3, zC2, zC3;             // Q**(r-3) and its z
     double zS2, zS3;                         // z of Q**(r-4)
 };
 
-// One tick.  A: the set of the newest y-interface so far, r-3/2 (its cell = Q*(r-1)); N: on entry its cell still
-// holds Q*(r-2) (from two ticks ago), on exit N is the set of interface r-1/2 (cell Q*(r)).
+// One tick.  The x-sweep works on row r of Q^n; the y-sweep and the source step run one row behind, on Q*(., ry),
+// ry = r-1, which the previous tick left in `cy.s*` -- so each phase between two barriers holds two independent
+// instruction streams (x and y) for the scheduler to interleave.
+// A: the set of the newest y-interface so far, ry-1/2 - 1 (its cell = Q*(ry-1)); N: on entry its cell still holds
+// Q*(ry-2) (from two ticks ago), on exit N is the set of interface ry-1/2 (cell Q*(ry)).
 template <int BX>
 __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th, Carry& cy, const YSet& A, YSet& N, int r,
                                      const RowMap rm, const RowMap rm_next, const double* __restrict__ q1,
                                      const double* __restrict__ q2, const double* __restrict__ q3,
                                      double* __restrict__ o1, double* __restrict__ o2, double* __restrict__ o3) {
-    // ---- this tick's cell of Q^n; prefetch the next row ------------------------------------------------------
+    const int ry = r - 1;
+    // ---- phase 0: this tick's cell of Q^n (prefetch the next row); y-cell of Q*(ry) ------------------------------
     double a1 = cy.n1, a2 = cy.n2, a3 = cy.n3;
     if (k.any_refl) {
         if (th.cm.neg2) a2 = -a2;
@@ -240,28 +259,40 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
         cy.n1 = q1[idx]; cy.n2 = q2[idx]; cy.n3 = q3[idx];
     }
     const bool row_in = r >= 0 && r < g.ny;
-
-    // ---- x-sweep of row r: cells -> waves -> limited fluxes -> Q*(., r)      (27)-(30), PAPER.md:159-198 ------
-    int tq = 0x7fffffff, td = 0x7fffffff;
+    int tq = 0x7fffffff, td = 0x7fffffff, tqy = 0x7fffffff, tdy = 0x7fffffff;
     const Cx cx = cell_of(a1, a2, a3, tq);
     sts2(th.p_cell, cx.q1, cx.q2); sts2(th.p_cell + 16, cx.q3, cx.hz2); sts1(th.p_cell + 32, cx.hz3);
+    const double b1o = N.c.q1, b2o = N.c.q2, b3o = N.c.q3;                    // Q*(ry-2), y-form (before N is overwritten)
+    N.c = cell_of(cy.s1, cy.s3, cy.s2, tqy);                                  // positions 2,3 switched
     __syncthreads();                                                          // B1: cells (and last tick's z) visible
+
+    // ---- phase 1: x-Riemann at i-1/2 of row r; y-Riemann at ry-1/2 ----------------------------------------------
     Cx L;
     {
         const double2 u0 = lds2(th.p_cell - SM_CELL), u1 = lds2(th.p_cell - SM_CELL + 16);
         L.q1 = u0.x; L.q2 = u0.y; L.q3 = u1.x; L.hz2 = u1.y; L.hz3 = lds1(th.p_cell - SM_CELL + 32);
     }
-    // d2x z of row r-3 (its z was published at the end of the previous tick)
-    double2 zW = lds2(th.p_z - SM_Z), zE = lds2(th.p_z + SM_Z);
+    double2 zW = lds2(th.p_z - SM_Z), zE = lds2(th.p_z + SM_Z);              // z of row ry-3, published last tick
     const Wv w = riemann2(L, cx, k.b2, k.omb2, td);
     const double rn1 = rnorm(w.s1, w.r31), rn2 = rnorm(w.s2, w.r32);
     sts2(th.p_wave, w.al1, w.s1); sts2(th.p_wave + 16, w.r31, w.al3); sts2(th.p_wave + 32, w.al2, w.s2);
     sts1(th.p_wave + 48, w.r32);
+    N.w = riemann2(A.c, N.c, k.b2, k.omb2, tdy);
+    N.rn1 = rnorm(N.w.s1, N.w.r31); N.rn2 = rnorm(N.w.s2, N.w.r32);
+    const double d1 = rdot(A.w.s1, A.w.r31, N.w.s1, N.w.r31), d2 = rdot(A.w.s2, A.w.r32, N.w.s2, N.w.r32);
+    N.pb1 = A.w.al1 * d1 * N.rn1; N.pb2 = A.w.al2 * d2 * N.rn2; N.pb3 = A.w.al3;      // if A is N's upwind side
+    const double hb1 = N.w.al1 * d1 * A.rn1, hb2 = N.w.al2 * d2 * A.rn2;              // if N is A's upwind side
     if (row_in) {
         th.mqx = min(th.mqx, tq); th.mdx = min(th.mdx, td);
-        th.smx = fmax(th.smx, fabs(hi_word(w.v) < 0 ? w.s2 : w.s1));          // max(|s1|,|s2|) = |v| + a
+        th.smx = dmax(th.smx, fabs(hi_word(w.v) < 0 ? w.s2 : w.s1));          // max(|s1|,|s2|) = |v| + a
+    }
+    if (ry >= k.j0 - 2 && ry >= -1 && ry <= g.ny + 1) {                       // y-interface ry-1/2 is one the scheme solves
+        th.mqy = min(th.mqy, tqy); th.mdy = min(th.mdy, tdy);
+        if (ry >= 0 && ry <= g.ny) th.smy = dmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
     }
     __syncthreads();                                                          // B2: waves visible
+
+    // ---- phase 2: limited fluxes of the x-interface i-1/2 and of the y-interface ry-3/2 (A) ----------------------
     Fl F;
     {
         const char* u1 = th.p_wave + (hi_word(w.s1) < 0 ? SM_WAVE : -SM_WAVE);   // upwind interface
@@ -274,46 +305,31 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
         F = flux2(w, b1, b2, k3, k.lamx);
     }
     sts2(th.p_gm, F.m1, F.m2); sts1(th.p_gm + 16, F.m3);
-    // source step, x part for row r-3 (independent of the barriers above; placed here to fill the wait)
-    if (th.fixW) zW = ghost_z(g, SIDE_XLO, (r - 3 + 0.5) * g.dy, -0.5 * g.dx, k.t, cy.zC2, cy.zC3);
-    if (th.fixE) zE = ghost_z(g, SIDE_XHI, (r - 3 + 0.5) * g.dy, (g.nx + 0.5) * g.dx, k.t, cy.zC2, cy.zC3);
-    const double H2 = fma(k.k2, cy.zC2, fma(k.kapx, zE.x + zW.x, cy.c2));
-    const double H3 = fma(k.k2, cy.zC3, fma(k.kapx, zE.y + zW.y, cy.c3));
-    __syncthreads();                                                          // B3: left-going parts visible
-    double s1, s2, s3;                                                        // Q*(i, r)
-    {
-        const double2 gm = lds2(th.p_gm + SM_GM);
-        const double gm3 = lds1(th.p_gm + SM_GM + 16);
-        s1 = fma(-k.lamx, F.p1 + gm.x, a1);
-        s2 = fma(-k.lamx, F.p2 + gm.y, a2);
-        s3 = fma(-k.lamx, F.p3 + gm3, a3);
-    }
-
-    // ---- y-sweep: interface r-1/2 (N), limited flux of interface r-3/2 (A), Q**(., r-2) ------------------------
-    const double b1o = N.c.q1, b2o = N.c.q2, b3o = N.c.q3;                    // Q*(r-2), y-form (before N is overwritten)
-    int tqy = 0x7fffffff, tdy = 0x7fffffff;
-    N.c = cell_of(s1, s3, s2, tqy);                                           // positions 2,3 switched
-    N.w = riemann2(A.c, N.c, k.b2, k.omb2, tdy);
-    N.rn1 = rnorm(N.w.s1, N.w.r31); N.rn2 = rnorm(N.w.s2, N.w.r32);
-    const double d1 = rdot(A.w.s1, A.w.r31, N.w.s1, N.w.r31), d2 = rdot(A.w.s2, A.w.r32, N.w.s2, N.w.r32);
-    N.pb1 = A.w.al1 * d1 * N.rn1; N.pb2 = A.w.al2 * d2 * N.rn2; N.pb3 = A.w.al3;      // if A is N's upwind side
-    const double hb1 = N.w.al1 * d1 * A.rn1, hb2 = N.w.al2 * d2 * A.rn2;              // if N is A's upwind side
     const Fl G = flux2(A.w, hi_word(A.w.s1) < 0 ? hb1 : A.pb1, hi_word(A.w.s2) < 0 ? hb2 : A.pb2,
                        hi_word(A.w.v) < 0 ? N.w.al3 : A.pb3, k.lamy);
-    const double n1 = fma(-k.lamy, cy.gp1 + G.m1, b1o);                       // Q**(i, r-2); physical order: n1, n2, n3
+    const double n1 = fma(-k.lamy, cy.gp1 + G.m1, b1o);                       // Q**(i, ry-2); physical order n1, n2, n3
     const double n3 = fma(-k.lamy, cy.gp2 + G.m2, b2o);
     const double n2 = fma(-k.lamy, cy.gp3 + G.m3, b3o);
     cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3;
-    if (r >= k.j0 - 2 && r >= -1 && r <= g.ny + 1) {                          // interface r-1/2 is one the scheme solves
-        th.mqy = min(th.mqy, tqy); th.mdy = min(th.mdy, tdy);
-        if (r >= 0 && r <= g.ny) th.smy = fmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
-    }
+    // source step, x part for row ry-3
+    if (th.fixW) zW = ghost_z(g, SIDE_XLO, (ry - 3 + 0.5) * g.dy, -0.5 * g.dx, k.t, cy.zC2, cy.zC3);
+    if (th.fixE) zE = ghost_z(g, SIDE_XHI, (ry - 3 + 0.5) * g.dy, (g.nx + 0.5) * g.dx, k.t, cy.zC2, cy.zC3);
+    const double H2 = fma(k.k2, cy.zC2, fma(k.kapx, zE.x + zW.x, cy.c2));
+    const double H3 = fma(k.k2, cy.zC3, fma(k.kapx, zE.y + zW.y, cy.c3));
+    __syncthreads();                                                          // B3: left-going parts visible
 
-    // ---- source step (26): publish z of row r-2, finish row R = r-3 ---------------------------------------------
+    // ---- phase 3: Q*(i, r) for the next tick; source step (26): publish z of row ry-2, finish row R = ry-3 -------
+    {
+        const double2 gm = lds2(th.p_gm + SM_GM);
+        const double gm3 = lds1(th.p_gm + SM_GM + 16);
+        cy.s1 = fma(-k.lamx, F.p1 + gm.x, a1);
+        cy.s2 = fma(-k.lamx, F.p2 + gm.y, a2);
+        cy.s3 = fma(-k.lamx, F.p3 + gm3, a3);
+    }
     const double rq = rcp_o1(n1);
     const double zN2 = n2 * rq, zN3 = n3 * rq;
     sts2(th.p_z, zN2, zN3);                                                   // read after B1 of the next tick
-    const int R = r - 3;
+    const int R = ry - 3;
     if (R >= k.j0) {                                                          // R < j1 by the loop bound
         double y2 = zN2 + cy.zS2, y3 = zN3 + cy.zS3;
         if (!k.py && (R == 0 || R == g.ny - 1)) {
@@ -378,10 +394,11 @@ __global__ void __launch_bounds__(BX, MINB) k_step_fused(Grid g, Clock* clk, con
     Y1 = Y0;
     Carry cy;
     cy.gp1 = cy.gp2 = cy.gp3 = 0.0;
+    cy.s1 = 1.0; cy.s2 = cy.s3 = 0.0;
     cy.c1 = 1.0; cy.c2 = cy.c3 = cy.zC2 = cy.zC3 = cy.zS2 = cy.zS3 = 0.0;
 
     int r = k.j0 - 3;
-    const int rend = k.j1 + 3;
+    const int rend = k.j1 + 4;                                     // the y-sweep and the source step run one row behind
     RowMap rm = map_row(g, r);
     {
         const size_t idx = (size_t)rm.row * g.nx + th.cm.col;
