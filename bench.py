@@ -28,7 +28,24 @@ if ROOT not in sys.path:
 
 METRIC = "fp64 Gcell-updates/s"
 UNIT = "Gcell-updates/s"
-ALG_BYTES_PER_CELL = 48.0          # 3 fields x 8 B x (1 read + 1 write) per cell-update (DESIGN.md "Rooflines")
+ALG_BYTES_PER_CELL = 48.0          # 3 fields x 8 B x (1 read + 1 write) per cell-update (DESIGN.md 7)
+ALG_FLOP_PER_CELL = 404.0          # the oracle's formulas, division / sqrt = 1
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 lanes x FMA x 1965 MHz = 37.2
+
+
+def reduce_max_ms(ms, dist, device):
+    """Max over ranks of a locally measured duration (the job is as slow as its slowest replica)."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(cells_per_replica, world, steps, ms):
+    """Gcell-updates/s of the whole job: every replica advances its own grid (replicas only, weak scaling)."""
+    return world * cells_per_replica * steps / (ms * 1e-3) / 1e9
 
 
 def make_workload(name):
@@ -239,11 +256,8 @@ def run_gpu(args):
     launches = s.kernel_launches() - l0
     clocks = sampler.stop(t_w0, t_w1)
     ms = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * w.cells * K / (ms * 1e-3) / 1e9
+    ms = reduce_max_ms(ms, dist, dev)
+    value = whole_job_value(w.cells, world, K, ms)
     names = {P.TIMED_STEP: "k_step_fused", P.TIMED_XSWEEP: "k_xsweep_unfused", P.TIMED_YSWEEP: "k_ysweep_unfused",
              P.TIMED_SOURCE: "k_source_unfused"}
     spans = {names[k]: s.kernel_time(k) for k in names}
@@ -262,9 +276,17 @@ def run_gpu(args):
     top_ms = spans[top][0] / spans[top][1]
     share = spans[top][0] / ms
     achieved = ALG_BYTES_PER_CELL * w.cells / (top_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": args.traffic, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": ALG_BYTES_PER_CELL * w.cells, "ms_per_launch": top_ms,
+    roofline_hbm = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": args.traffic, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": ALG_BYTES_PER_CELL * w.cells}
+    tf = ALG_FLOP_PER_CELL * w.cells / (top_ms * 1e-3) / 1e12
+    sm_mhz = clocks.get("sm_mhz") or 1965.0
+    roofline = {"bound": "alu", "kernel": top, "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": tf / FP64_PEAK_TFLOPS, "traffic": args.traffic,
+                "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x 1.965 GHz (DESIGN.md 7); fp64 vector pipe, "
+                               "not in MEASURED_PEAKS.json",
+                "frac_at_observed_clock": tf / (FP64_PEAK_TFLOPS * sm_mhz / 1965.0),
+                "algorithmic_flop_per_launch": ALG_FLOP_PER_CELL * w.cells, "ms_per_launch": top_ms,
                 "share_of_step": share,
                 "kernels": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1]} for k, v in spans.items()}}
 
@@ -306,7 +328,7 @@ def run_gpu(args):
                    "l2": "state larger than L2, no flush" if 24 * w.cells > 4 * 126e6 else "state near/below L2 size",
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "flags": int(flags),
                    "t_end_s": info["t"], "last_cfl": info["cfl"]},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_hbm": roofline_hbm,
         "cpu_baseline": base,
     }
     print(json.dumps(out))
