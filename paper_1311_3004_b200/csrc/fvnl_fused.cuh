@@ -196,9 +196,12 @@ struct YSet {
     double pb1, pb2, pb3;
 };
 
-// Shared-memory layout: one record per column, strides chosen as odd multiples of 16 B so that 128-bit accesses
-// of consecutive columns are bank-conflict free; one pad record on each side so that tid-1 / tid+1 never clamp.
-constexpr int SM_CELL = 48, SM_WAVE = 80, SM_GM = 48, SM_Z = 16;
+// Shared-memory layout: ten arrays of double2, one element per column (+ one pad element on each side so that
+// tid-1 / tid+1 never clamp).  Every access is [p + constant] from ONE per-thread pointer p = base + 16 (tid+1);
+// 128-bit accesses of consecutive columns are bank-conflict free.
+//   0 (q1,q2)  1 (q3,hz2)  2 (hz3,-)  3 (al1,s1)  4 (r31,al3)  5 (al2,s2)  6 (r32,-)  7 (m1,m2)  8 (m3,-)  9 (z2,z3)
+constexpr int SM_ARRAYS = 10;
+template <int BX> __host__ __device__ constexpr int sm_off(int k) { return k * (BX + 2) * 16; }
 
 __device__ __forceinline__ void sts2(char* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
 __device__ __forceinline__ double2 lds2(const char* p) { return *reinterpret_cast<const double2*>(p); }
@@ -210,6 +213,7 @@ struct StepK {
     double t, lamx, lamy, kapx, kapy, k2;    // k2 = -2 (kapx + kapy)
     double b2, omb2;                         // 2 (beta - 1), 1 - b2
     int j0, j1;                              // rows of output of this chunk: [j0, j1)
+    int ylo, ycnt;                           // y-interface ry-1/2 is one the scheme solves iff (unsigned)(ry-ylo) <= ycnt
     bool px, py, any_src, any_refl;
 };
 
@@ -217,8 +221,9 @@ struct StepK {
 struct ThreadK {
     ColMap cm;
     int i;                                   // column on the ghost-extended mesh
-    bool fixW, fixE, out_col;
-    char *p_cell, *p_wave, *p_gm, *p_z;      // this column's shared-memory records
+    bool out_col;
+    char* p;                                 // this column's element of the shared-memory arrays
+    int special;                             // bit 0: fixW, bit 1: fixE (source-step ghosts at the x edges)
     // running reductions (masked by validity at the end)
     double smx, smy;
     int mqx, mdx, mqy, mdy, mxo;             // min high words of q1 / disc in x and y; max |high word| of the output
@@ -258,10 +263,11 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
         const size_t idx = (size_t)rm_next.row * g.nx + th.cm.col;
         cy.n1 = q1[idx]; cy.n2 = q2[idx]; cy.n3 = q3[idx];
     }
-    const bool row_in = r >= 0 && r < g.ny;
+    const bool row_in = (unsigned)r < (unsigned)g.ny;
     int tq = 0x7fffffff, td = 0x7fffffff, tqy = 0x7fffffff, tdy = 0x7fffffff;
     const Cx cx = cell_of(a1, a2, a3, tq);
-    sts2(th.p_cell, cx.q1, cx.q2); sts2(th.p_cell + 16, cx.q3, cx.hz2); sts1(th.p_cell + 32, cx.hz3);
+    char* const p = th.p;
+    sts2(p + sm_off<BX>(0), cx.q1, cx.q2); sts2(p + sm_off<BX>(1), cx.q3, cx.hz2); sts1(p + sm_off<BX>(2), cx.hz3);
     const double b1o = N.c.q1, b2o = N.c.q2, b3o = N.c.q3;                    // Q*(ry-2), y-form (before N is overwritten)
     N.c = cell_of(cy.s1, cy.s3, cy.s2, tqy);                                  // positions 2,3 switched
     __syncthreads();                                                          // B1: cells (and last tick's z) visible
@@ -269,14 +275,14 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
     // ---- phase 1: x-Riemann at i-1/2 of row r; y-Riemann at ry-1/2 ----------------------------------------------
     Cx L;
     {
-        const double2 u0 = lds2(th.p_cell - SM_CELL), u1 = lds2(th.p_cell - SM_CELL + 16);
-        L.q1 = u0.x; L.q2 = u0.y; L.q3 = u1.x; L.hz2 = u1.y; L.hz3 = lds1(th.p_cell - SM_CELL + 32);
+        const double2 u0 = lds2(p + sm_off<BX>(0) - 16), u1 = lds2(p + sm_off<BX>(1) - 16);
+        L.q1 = u0.x; L.q2 = u0.y; L.q3 = u1.x; L.hz2 = u1.y; L.hz3 = lds1(p + sm_off<BX>(2) - 16);
     }
-    double2 zW = lds2(th.p_z - SM_Z), zE = lds2(th.p_z + SM_Z);              // z of row ry-3, published last tick
+    double2 zW = lds2(p + sm_off<BX>(9) - 16), zE = lds2(p + sm_off<BX>(9) + 16);   // z of row ry-3, published last tick
     const Wv w = riemann2(L, cx, k.b2, k.omb2, td);
     const double rn1 = rnorm(w.s1, w.r31), rn2 = rnorm(w.s2, w.r32);
-    sts2(th.p_wave, w.al1, w.s1); sts2(th.p_wave + 16, w.r31, w.al3); sts2(th.p_wave + 32, w.al2, w.s2);
-    sts1(th.p_wave + 48, w.r32);
+    sts2(p + sm_off<BX>(3), w.al1, w.s1); sts2(p + sm_off<BX>(4), w.r31, w.al3); sts2(p + sm_off<BX>(5), w.al2, w.s2);
+    sts1(p + sm_off<BX>(6), w.r32);
     N.w = riemann2(A.c, N.c, k.b2, k.omb2, tdy);
     N.rn1 = rnorm(N.w.s1, N.w.r31); N.rn2 = rnorm(N.w.s2, N.w.r32);
     const double d1 = rdot(A.w.s1, A.w.r31, N.w.s1, N.w.r31), d2 = rdot(A.w.s2, A.w.r32, N.w.s2, N.w.r32);
@@ -286,25 +292,25 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
         th.mqx = min(th.mqx, tq); th.mdx = min(th.mdx, td);
         th.smx = dmax(th.smx, fabs(hi_word(w.v) < 0 ? w.s2 : w.s1));          // max(|s1|,|s2|) = |v| + a
     }
-    if (ry >= k.j0 - 2 && ry >= -1 && ry <= g.ny + 1) {                       // y-interface ry-1/2 is one the scheme solves
+    if ((unsigned)(ry - k.ylo) <= (unsigned)k.ycnt) {                         // y-interface ry-1/2 is one the scheme solves
         th.mqy = min(th.mqy, tqy); th.mdy = min(th.mdy, tdy);
-        if (ry >= 0 && ry <= g.ny) th.smy = dmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
+        if ((unsigned)ry <= (unsigned)g.ny) th.smy = dmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
     }
     __syncthreads();                                                          // B2: waves visible
 
     // ---- phase 2: limited fluxes of the x-interface i-1/2 and of the y-interface ry-3/2 (A) ----------------------
     Fl F;
     {
-        const char* u1 = th.p_wave + (hi_word(w.s1) < 0 ? SM_WAVE : -SM_WAVE);   // upwind interface
-        const char* u2 = th.p_wave + (hi_word(w.s2) < 0 ? SM_WAVE : -SM_WAVE);
-        const char* u3 = th.p_wave + (hi_word(w.v) < 0 ? SM_WAVE : -SM_WAVE);
-        const double2 k1 = lds2(u1), k2 = lds2(u2 + 32);
-        const double k1r = lds1(u1 + 16), k2r = lds1(u2 + 48), k3 = lds1(u3 + 24);
+        const char* u1 = p + (hi_word(w.s1) < 0 ? 16 : -16);                  // upwind interface
+        const char* u2 = p + (hi_word(w.s2) < 0 ? 16 : -16);
+        const char* u3 = p + (hi_word(w.v) < 0 ? 16 : -16);
+        const double2 k1 = lds2(u1 + sm_off<BX>(3)), k2 = lds2(u2 + sm_off<BX>(5));
+        const double k1r = lds1(u1 + sm_off<BX>(4)), k2r = lds1(u2 + sm_off<BX>(6)), k3 = lds1(u3 + sm_off<BX>(4) + 8);
         const double b1 = k1.x * rdot(k1.y, k1r, w.s1, w.r31) * rn1;
         const double b2 = k2.x * rdot(k2.y, k2r, w.s2, w.r32) * rn2;
         F = flux2(w, b1, b2, k3, k.lamx);
     }
-    sts2(th.p_gm, F.m1, F.m2); sts1(th.p_gm + 16, F.m3);
+    sts2(p + sm_off<BX>(7), F.m1, F.m2); sts1(p + sm_off<BX>(8), F.m3);
     const Fl G = flux2(A.w, hi_word(A.w.s1) < 0 ? hb1 : A.pb1, hi_word(A.w.s2) < 0 ? hb2 : A.pb2,
                        hi_word(A.w.v) < 0 ? N.w.al3 : A.pb3, k.lamy);
     const double n1 = fma(-k.lamy, cy.gp1 + G.m1, b1o);                       // Q**(i, ry-2); physical order n1, n2, n3
@@ -312,23 +318,25 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
     const double n2 = fma(-k.lamy, cy.gp3 + G.m3, b3o);
     cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3;
     // source step, x part for row ry-3
-    if (th.fixW) zW = ghost_z(g, SIDE_XLO, (ry - 3 + 0.5) * g.dy, -0.5 * g.dx, k.t, cy.zC2, cy.zC3);
-    if (th.fixE) zE = ghost_z(g, SIDE_XHI, (ry - 3 + 0.5) * g.dy, (g.nx + 0.5) * g.dx, k.t, cy.zC2, cy.zC3);
+    if (th.special) {
+        if (th.special & 1) zW = ghost_z(g, SIDE_XLO, (ry - 3 + 0.5) * g.dy, -0.5 * g.dx, k.t, cy.zC2, cy.zC3);
+        if (th.special & 2) zE = ghost_z(g, SIDE_XHI, (ry - 3 + 0.5) * g.dy, (g.nx + 0.5) * g.dx, k.t, cy.zC2, cy.zC3);
+    }
     const double H2 = fma(k.k2, cy.zC2, fma(k.kapx, zE.x + zW.x, cy.c2));
     const double H3 = fma(k.k2, cy.zC3, fma(k.kapx, zE.y + zW.y, cy.c3));
     __syncthreads();                                                          // B3: left-going parts visible
 
     // ---- phase 3: Q*(i, r) for the next tick; source step (26): publish z of row ry-2, finish row R = ry-3 -------
     {
-        const double2 gm = lds2(th.p_gm + SM_GM);
-        const double gm3 = lds1(th.p_gm + SM_GM + 16);
+        const double2 gm = lds2(p + sm_off<BX>(7) + 16);
+        const double gm3 = lds1(p + sm_off<BX>(8) + 16);
         cy.s1 = fma(-k.lamx, F.p1 + gm.x, a1);
         cy.s2 = fma(-k.lamx, F.p2 + gm.y, a2);
         cy.s3 = fma(-k.lamx, F.p3 + gm3, a3);
     }
     const double rq = rcp_o1(n1);
     const double zN2 = n2 * rq, zN3 = n3 * rq;
-    sts2(th.p_z, zN2, zN3);                                                   // read after B1 of the next tick
+    sts2(p + sm_off<BX>(9), zN2, zN3);                                        // read after B1 of the next tick
     const int R = ry - 3;
     if (R >= k.j0) {                                                          // R < j1 by the loop bound
         double y2 = zN2 + cy.zS2, y3 = zN3 + cy.zS3;
@@ -351,7 +359,7 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
 }
 
 template <int BX>
-__host__ __device__ constexpr int fused_smem_bytes() { return (BX + 2) * (SM_CELL + SM_WAVE + SM_GM + SM_Z); }
+__host__ __device__ constexpr int fused_smem_bytes() { return sm_off<BX>(SM_ARRAYS); }
 
 // The step kernel.  grid = (strips, chunks); block = BX threads; dynamic shared memory = fused_smem_bytes<BX>().
 // rows: rows of output per chunk.
@@ -369,6 +377,7 @@ __global__ void __launch_bounds__(BX, MINB) k_step_fused(Grid g, Clock* clk, con
     k.k2 = -2.0 * (k.kapx + k.kapy);
     k.b2 = 2.0 * (g.beta - 1.0); k.omb2 = 1.0 - k.b2;
     k.j0 = (int)blockIdx.y * rows; k.j1 = min(k.j0 + rows, g.ny);
+    k.ylo = max(k.j0 - 2, -1); k.ycnt = g.ny + 1 - k.ylo;
     k.px = g.side[SIDE_XLO].kind == BC_PERIODIC; k.py = g.side[SIDE_YLO].kind == BC_PERIODIC;
     k.any_src = g.side[0].kind == BC_SOURCE || g.side[1].kind == BC_SOURCE || g.side[2].kind == BC_SOURCE ||
                 g.side[3].kind == BC_SOURCE;
@@ -378,12 +387,9 @@ __global__ void __launch_bounds__(BX, MINB) k_step_fused(Grid g, Clock* clk, con
     ThreadK th;
     th.i = (int)blockIdx.x * (BX - 6) - 3 + tid;
     th.cm = map_column(g, th.i);
-    th.fixW = !k.px && th.i == 0; th.fixE = !k.px && th.i == g.nx - 1;
+    th.special = (!k.px && th.i == 0 ? 1 : 0) | (!k.px && th.i == g.nx - 1 ? 2 : 0);
     th.out_col = tid >= 3 && tid <= BX - 4 && th.i >= 0 && th.i < g.nx;
-    th.p_cell = smem + (tid + 1) * SM_CELL;
-    th.p_wave = smem + (BX + 2) * SM_CELL + (tid + 1) * SM_WAVE;
-    th.p_gm = smem + (BX + 2) * (SM_CELL + SM_WAVE) + (tid + 1) * SM_GM;
-    th.p_z = smem + (BX + 2) * (SM_CELL + SM_WAVE + SM_GM) + (tid + 1) * SM_Z;
+    th.p = smem + (tid + 1) * 16;
     th.smx = 0.0; th.smy = 0.0;
     th.mqx = th.mdx = th.mqy = th.mdy = 0x7fffffff; th.mxo = 0;
 
