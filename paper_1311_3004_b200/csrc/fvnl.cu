@@ -326,24 +326,32 @@ static int ensure_star(fvnl_ctx* c) {
 struct FusedVariant { int bx, minb; };
 static const FusedVariant FUSED_VARIANTS[] = {{128, 3}, {256, 2}, {128, 4}, {256, 1}};
 
-static int fused_rows(const fvnl_ctx* c, int strips) {
-    if (c->rows_per_block > 0) return c->rows_per_block < c->g.ny ? c->rows_per_block : c->g.ny;
-    // enough blocks to fill the machine several times over, chunks not shorter than 64 rows (6 halo rows each)
+// Rows per chunk.  All blocks do the same work, so the grid runs as "waves" of `slots` resident blocks: pick the
+// number of chunks that maximises  (work in full waves) x (useful rows per marched row):
+//     efficiency = blocks / (ceil(blocks / slots) * slots)  *  rows / (rows + 7)
+// (7 = the pipeline fill of a chunk: 3 halo rows below, 3 above, 1 for the y-sweep running one row behind).
+static int fused_rows(const fvnl_ctx* c, int strips, int slots) {
     const int ny = c->g.ny;
-    const int want_blocks = 148 * 4 * 6;
-    int chunks = (want_blocks + strips - 1) / strips;
-    int rows = (ny + chunks - 1) / chunks;
-    if (rows < 64) rows = 64;
-    if (rows > 512) rows = 512;
-    if (rows > ny) rows = ny;
-    return rows;
+    if (c->rows_per_block > 0) return c->rows_per_block < ny ? c->rows_per_block : ny;
+    int best_rows = ny;
+    double best = -1.0;
+    const int max_chunks = ny / 16 > 0 ? ny / 16 : 1;               // chunks not shorter than 16 rows
+    for (int chunks = 1; chunks <= max_chunks && chunks <= 4096; ++chunks) {
+        const int rows = (ny + chunks - 1) / chunks;
+        const int nch = (ny + rows - 1) / rows;
+        const long blocks = (long)strips * nch;
+        const long waves = (blocks + slots - 1) / slots;
+        const double eff = (double)blocks / (double)(waves * slots) * rows / (rows + 7.0);
+        if (eff > best + 1e-9) { best = eff; best_rows = rows; }
+    }
+    return best_rows;
 }
 
 template <int BX, int MINB>
 static void launch_fused_t(fvnl_ctx* c, double** a, double** b) {
     const Grid& g = c->g;
     const int strips = (g.nx + (BX - 6) - 1) / (BX - 6);
-    const int rows = fused_rows(c, strips);
+    const int rows = fused_rows(c, strips, 148 * MINB);
     const dim3 grd(strips, (g.ny + rows - 1) / rows);
     static bool attr_set = false;
     if (!attr_set) {
@@ -356,9 +364,9 @@ static void launch_fused_t(fvnl_ctx* c, double** a, double** b) {
 
 static void launch_fused(fvnl_ctx* c, double** a, double** b) {
     switch (c->variant) {
-        case 1: launch_fused_t<256, 2>(c, a, b); break;
-        case 2: launch_fused_t<128, 4>(c, a, b); break;
-        case 3: launch_fused_t<256, 1>(c, a, b); break;
+        case 1: launch_fused_t<160, 3>(c, a, b); break;
+        case 2: launch_fused_t<96, 5>(c, a, b); break;
+        case 3: launch_fused_t<64, 7>(c, a, b); break;
         default: launch_fused_t<128, 3>(c, a, b); break;
     }
 }

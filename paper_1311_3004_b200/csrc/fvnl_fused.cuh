@@ -288,6 +288,12 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
     const double d1 = rdot(A.w.s1, A.w.r31, N.w.s1, N.w.r31), d2 = rdot(A.w.s2, A.w.r32, N.w.s2, N.w.r32);
     N.pb1 = A.w.al1 * d1 * N.rn1; N.pb2 = A.w.al2 * d2 * N.rn2; N.pb3 = A.w.al3;      // if A is N's upwind side
     const double hb1 = N.w.al1 * d1 * A.rn1, hb2 = N.w.al2 * d2 * A.rn2;              // if N is A's upwind side
+    const Fl G = flux2(A.w, hi_word(A.w.s1) < 0 ? hb1 : A.pb1, hi_word(A.w.s2) < 0 ? hb2 : A.pb2,
+                       hi_word(A.w.v) < 0 ? N.w.al3 : A.pb3, k.lamy);
+    const double n1 = fma(-k.lamy, cy.gp1 + G.m1, b1o);                       // Q**(i, ry-2); physical order n1, n2, n3
+    const double n3 = fma(-k.lamy, cy.gp2 + G.m2, b2o);
+    const double n2 = fma(-k.lamy, cy.gp3 + G.m3, b3o);
+    cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3;
     if (row_in) {
         th.mqx = min(th.mqx, tq); th.mdx = min(th.mdx, td);
         th.smx = dmax(th.smx, fabs(hi_word(w.v) < 0 ? w.s2 : w.s1));          // max(|s1|,|s2|) = |v| + a
@@ -311,12 +317,6 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
         F = flux2(w, b1, b2, k3, k.lamx);
     }
     sts2(p + sm_off<BX>(7), F.m1, F.m2); sts1(p + sm_off<BX>(8), F.m3);
-    const Fl G = flux2(A.w, hi_word(A.w.s1) < 0 ? hb1 : A.pb1, hi_word(A.w.s2) < 0 ? hb2 : A.pb2,
-                       hi_word(A.w.v) < 0 ? N.w.al3 : A.pb3, k.lamy);
-    const double n1 = fma(-k.lamy, cy.gp1 + G.m1, b1o);                       // Q**(i, ry-2); physical order n1, n2, n3
-    const double n3 = fma(-k.lamy, cy.gp2 + G.m2, b2o);
-    const double n2 = fma(-k.lamy, cy.gp3 + G.m3, b3o);
-    cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3;
     // source step, x part for row ry-3
     if (th.special) {
         if (th.special & 1) zW = ghost_z(g, SIDE_XLO, (ry - 3 + 0.5) * g.dy, -0.5 * g.dx, k.t, cy.zC2, cy.zC3);
