@@ -208,6 +208,17 @@ __device__ __forceinline__ double2 lds2(const char* p) { return *reinterpret_cas
 __device__ __forceinline__ void sts1(char* p, double a) { *reinterpret_cast<double*>(p) = a; }
 __device__ __forceinline__ double lds1(const char* p) { return *reinterpret_cast<const double*>(p); }
 
+// Rows of Q^n are prefetched two ticks ahead with cp.async (LDGSTS) into a four-slot ring of shared memory, each
+// thread copying and later reading only its own three values -- no barrier needed, no registers held by loads in
+// flight, and the compiler cannot sink the loads towards their use.
+__device__ __forceinline__ void cp_async8(char* smem_dst, const double* gsrc) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+template <int BX> __host__ __device__ constexpr int pre_slot_bytes() { return 3 * BX * 8; }
+
 // Block-invariant quantities of a step.
 struct StepK {
     double t, lamx, lamy, kapx, kapy, k2;    // k2 = -2 (kapx + kapy)
@@ -223,7 +234,9 @@ struct ThreadK {
     int i;                                   // column on the ghost-extended mesh
     bool out_col;
     char* p;                                 // this column's element of the shared-memory arrays
-    int special;                             // bit 0: fixW, bit 1: fixE (source-step ghosts at the x edges)
+    char* pq;                                // this column's element of slot 0 / field 0 of the prefetch ring
+    int special;                             // bit 0: fixW, bit 1: fixE (source-step ghosts at the x edges),
+                                             // bit 2: ghost column of a REFLECT side, bit 3: of a SOURCE side
     // running reductions (masked by validity at the end)
     double smx, smy;
     int mqx, mdx, mqy, mdy, mxo;             // min high words of q1 / disc in x and y; max |high word| of the output
@@ -231,7 +244,6 @@ struct ThreadK {
 
 // Carried between ticks besides the two YSets.
 struct Carry {
-    double n1, n2, n3;                       // prefetched row r+1 of Q^n
     double s1, s2, s3;                       // Q*(., r-1), left by the previous tick for the y-sweep
     double gp1, gp2, gp3;                    // right-going part of the y-interface below the newest one, y-form
     double c1, c2, c3, zC2, zC3;             // Q**(r-3) and its z
@@ -243,27 +255,43 @@ struct Carry {
 // instruction streams (x and y) for the scheduler to interleave.
 // A: the set of the newest y-interface so far, ry-1/2 - 1 (its cell = Q*(ry-1)); N: on entry its cell still holds
 // Q*(ry-2) (from two ticks ago), on exit N is the set of interface ry-1/2 (cell Q*(ry)).
-template <int BX>
+// STEADY: the tick is in the steady part of the march of an interior stretch of rows -- every row it touches is an
+// interior row, every pipeline stage holds real data and writes output, no y-edge is near; then all the per-tick
+// conditions are known at compile time (the kernel runs the few other ticks of a chunk with STEADY = false).
+template <int BX, bool STEADY>
 __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th, Carry& cy, const YSet& A, YSet& N, int r,
-                                     const RowMap rm, const RowMap rm_next, const double* __restrict__ q1,
+                                     const double* __restrict__ q1,
                                      const double* __restrict__ q2, const double* __restrict__ q3,
                                      double* __restrict__ o1, double* __restrict__ o2, double* __restrict__ o3) {
     const int ry = r - 1;
-    // ---- phase 0: this tick's cell of Q^n (prefetch the next row); y-cell of Q*(ry) ------------------------------
-    double a1 = cy.n1, a2 = cy.n2, a3 = cy.n3;
-    if (k.any_refl) {
-        if (th.cm.neg2) a2 = -a2;
-        if (rm.neg3) a3 = -a3;
+    RowMap rm, rm_pre;                                                        // rows r and r+2 (the one to prefetch)
+    if (STEADY) {
+        rm.row = r; rm.neg3 = false; rm.ysrc = -1;
+        rm_pre.row = r + 2;
+    } else {
+        rm = map_row(g, r);
+        rm_pre = map_row(g, r + 2);
     }
-    if (k.any_src && (th.cm.xsrc >= 0 || rm.ysrc >= 0)) {
-        const double3 s = apply_sources(g, th.cm.xsrc, rm.ysrc, th.cm.col, th.cm.neg2, th.i, r, k.t, a1, a2, a3);
-        a1 = s.x; a2 = s.y; a3 = s.z;
-    }
+    // ---- phase 0: this tick's cell of Q^n (prefetch row r+2); y-cell of Q*(ry) ------------------------------------
+    cp_async_wait<1>();                                                       // row r has landed (row r+1 may be in flight)
+    double a1, a2, a3;
     {
-        const size_t idx = (size_t)rm_next.row * g.nx + th.cm.col;
-        cy.n1 = q1[idx]; cy.n2 = q2[idx]; cy.n3 = q3[idx];
+        const char* ps = th.pq + (r & 3) * pre_slot_bytes<BX>();
+        a1 = lds1(ps); a2 = lds1(ps + BX * 8); a3 = lds1(ps + 2 * BX * 8);
+        char* pd = th.pq + ((r + 2) & 3) * pre_slot_bytes<BX>();
+        const size_t idx = (size_t)rm_pre.row * g.nx + th.cm.col;
+        cp_async8(pd, q1 + idx); cp_async8(pd + BX * 8, q2 + idx); cp_async8(pd + 2 * BX * 8, q3 + idx);
+        cp_async_commit();
     }
-    const bool row_in = (unsigned)r < (unsigned)g.ny;
+    if (!STEADY && rm.neg3) a3 = -a3;
+    if ((th.special & 12) || (!STEADY && rm.ysrc >= 0)) {                     // ghost column of a REFLECT / SOURCE side,
+        if (th.special & 4) a2 = -a2;                                         // ghost row of a SOURCE side: rare
+        if ((th.special & 8) || rm.ysrc >= 0) {
+            const double3 s = apply_sources(g, th.cm.xsrc, rm.ysrc, th.cm.col, th.cm.neg2, th.i, r, k.t, a1, a2, a3);
+            a1 = s.x; a2 = s.y; a3 = s.z;
+        }
+    }
+    const bool row_in = STEADY || (unsigned)r < (unsigned)g.ny;
     int tq = 0x7fffffff, td = 0x7fffffff, tqy = 0x7fffffff, tdy = 0x7fffffff;
     const Cx cx = cell_of(a1, a2, a3, tq);
     char* const p = th.p;
@@ -298,9 +326,9 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
         th.mqx = min(th.mqx, tq); th.mdx = min(th.mdx, td);
         th.smx = dmax(th.smx, fabs(hi_word(w.v) < 0 ? w.s2 : w.s1));          // max(|s1|,|s2|) = |v| + a
     }
-    if ((unsigned)(ry - k.ylo) <= (unsigned)k.ycnt) {                         // y-interface ry-1/2 is one the scheme solves
+    if (STEADY || (unsigned)(ry - k.ylo) <= (unsigned)k.ycnt) {               // y-interface ry-1/2 is one the scheme solves
         th.mqy = min(th.mqy, tqy); th.mdy = min(th.mdy, tdy);
-        if ((unsigned)ry <= (unsigned)g.ny) th.smy = dmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
+        if (STEADY || (unsigned)ry <= (unsigned)g.ny) th.smy = dmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
     }
     __syncthreads();                                                          // B2: waves visible
 
@@ -318,7 +346,7 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
     }
     sts2(p + sm_off<BX>(7), F.m1, F.m2); sts1(p + sm_off<BX>(8), F.m3);
     // source step, x part for row ry-3
-    if (th.special) {
+    if (th.special & 3) {
         if (th.special & 1) zW = ghost_z(g, SIDE_XLO, (ry - 3 + 0.5) * g.dy, -0.5 * g.dx, k.t, cy.zC2, cy.zC3);
         if (th.special & 2) zE = ghost_z(g, SIDE_XHI, (ry - 3 + 0.5) * g.dy, (g.nx + 0.5) * g.dx, k.t, cy.zC2, cy.zC3);
     }
@@ -338,9 +366,9 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
     const double zN2 = n2 * rq, zN3 = n3 * rq;
     sts2(p + sm_off<BX>(9), zN2, zN3);                                        // read after B1 of the next tick
     const int R = ry - 3;
-    if (R >= k.j0) {                                                          // R < j1 by the loop bound
+    if (STEADY || R >= k.j0) {                                                // R < j1 by the loop bound
         double y2 = zN2 + cy.zS2, y3 = zN3 + cy.zS3;
-        if (!k.py && (R == 0 || R == g.ny - 1)) {
+        if (!STEADY && !k.py && (R == 0 || R == g.ny - 1)) {
             const double x = (th.i + 0.5) * g.dx;
             double2 lo = make_double2(cy.zS2, cy.zS3), hi = make_double2(zN2, zN3);
             if (R == 0) lo = ghost_z(g, SIDE_YLO, x, x, k.t, cy.zC2, cy.zC3);
@@ -359,12 +387,14 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
 }
 
 template <int BX>
-__host__ __device__ constexpr int fused_smem_bytes() { return sm_off<BX>(SM_ARRAYS); }
+__host__ __device__ constexpr int fused_smem_bytes() { return sm_off<BX>(SM_ARRAYS) + 4 * pre_slot_bytes<BX>(); }
 
 // The step kernel.  grid = (strips, chunks); block = BX threads; dynamic shared memory = fused_smem_bytes<BX>().
 // rows: rows of output per chunk.
+// MINB: blocks per SM the register budget is set for (65536 registers / (BX * MINB) per thread, multiple of 8).
 template <int BX, int MINB>
-__global__ void __launch_bounds__(BX, MINB) k_step_fused(Grid g, Clock* clk, const double* __restrict__ q1,
+__global__ void __launch_bounds__(BX) __maxnreg__((65536 / (BX * MINB)) / 8 * 8 > 255 ? 255 : (65536 / (BX * MINB)) / 8 * 8)
+k_step_fused(Grid g, Clock* clk, const double* __restrict__ q1,
                                                          const double* __restrict__ q2, const double* __restrict__ q3,
                                                          double* __restrict__ o1, double* __restrict__ o2,
                                                          double* __restrict__ o3, int rows) {
@@ -387,9 +417,11 @@ __global__ void __launch_bounds__(BX, MINB) k_step_fused(Grid g, Clock* clk, con
     ThreadK th;
     th.i = (int)blockIdx.x * (BX - 6) - 3 + tid;
     th.cm = map_column(g, th.i);
-    th.special = (!k.px && th.i == 0 ? 1 : 0) | (!k.px && th.i == g.nx - 1 ? 2 : 0);
+    th.special = (!k.px && th.i == 0 ? 1 : 0) | (!k.px && th.i == g.nx - 1 ? 2 : 0) | (th.cm.neg2 ? 4 : 0) |
+                 (th.cm.xsrc >= 0 ? 8 : 0);
     th.out_col = tid >= 3 && tid <= BX - 4 && th.i >= 0 && th.i < g.nx;
     th.p = smem + (tid + 1) * 16;
+    th.pq = smem + sm_off<BX>(SM_ARRAYS) + tid * 8;
     th.smx = 0.0; th.smy = 0.0;
     th.mqx = th.mdx = th.mqy = th.mdy = 0x7fffffff; th.mxo = 0;
 
@@ -405,21 +437,32 @@ __global__ void __launch_bounds__(BX, MINB) k_step_fused(Grid g, Clock* clk, con
 
     int r = k.j0 - 3;
     const int rend = k.j1 + 4;                                     // the y-sweep and the source step run one row behind
-    RowMap rm = map_row(g, r);
-    {
+    __syncthreads();                                               // (the zero fill above is complete)
+    for (int d = 0; d < 2; ++d) {                                  // rows r and r+1 start their way into the ring
+        const RowMap rm = map_row(g, r + d);
         const size_t idx = (size_t)rm.row * g.nx + th.cm.col;
-        cy.n1 = q1[idx]; cy.n2 = q2[idx]; cy.n3 = q3[idx];
+        char* pd = th.pq + ((r + d) & 3) * pre_slot_bytes<BX>();
+        cp_async8(pd, q1 + idx); cp_async8(pd + BX * 8, q2 + idx); cp_async8(pd + 2 * BX * 8, q3 + idx);
+        cp_async_commit();
     }
-    __syncthreads();
-    while (true) {
-        RowMap rmn = map_row(g, r + 1);
-        tick<BX>(g, k, th, cy, Y0, Y1, r, rm, rmn, q1, q2, q3, o1, o2, o3);
-        if (++r >= rend) break;
-        rm = map_row(g, r + 1);
-        tick<BX>(g, k, th, cy, Y1, Y0, r, rmn, rm, q1, q2, q3, o1, o2, o3);
-        if (++r >= rend) break;
+    // steady ticks: r in [slo, shi] (see tick<>): rows r, r+1 interior; output row r-4 >= j0, away from the y edges
+    const int slo = max(k.j0 + 4, k.py ? 0 : 5), shi = min(rend - 1, g.ny - 3);
+    while (r < rend && r < slo) {                                  // pipeline fill (and everything, near the y edges)
+        tick<BX, false>(g, k, th, cy, Y0, Y1, r, q1, q2, q3, o1, o2, o3);
+        const YSet t = Y0; Y0 = Y1; Y1 = t;
+        ++r;
+    }
+    for (; r + 1 <= shi; r += 2) {
+        tick<BX, true>(g, k, th, cy, Y0, Y1, r, q1, q2, q3, o1, o2, o3);
+        tick<BX, true>(g, k, th, cy, Y1, Y0, r + 1, q1, q2, q3, o1, o2, o3);
+    }
+    while (r < rend) {
+        tick<BX, false>(g, k, th, cy, Y0, Y1, r, q1, q2, q3, o1, o2, o3);
+        const YSet t = Y0; Y0 = Y1; Y1 = t;
+        ++r;
     }
 
+    cp_async_wait<0>();
     // ---- reductions: M of and the sticky flags, masked by which results of this thread are real ----
     const int i = th.i;
     const bool x_if_m = tid >= 1 && i >= 0 && i <= g.nx;            // x-interface i-1/2 touches an interior cell
