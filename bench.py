@@ -222,7 +222,7 @@ def run_gpu(args):
         s.set_bc(side, kind, src)
     if args.kernel == "unfused":
         s.set_option(P.OPT_KERNEL, P.KERNEL_UNFUSED)
-    if args.variant:
+    if args.variant >= 0:
         s.set_option(P.OPT_VARIANT, args.variant)
     if args.rows:
         s.set_option(P.OPT_ROWS_PER_BLOCK, args.rows)
@@ -346,7 +346,7 @@ def main():
     ap.add_argument("--workload", default="C5-16384")
     ap.add_argument("--kernel", default="fused", choices=["fused", "unfused"])
     ap.add_argument("--e2e-steps", type=int, default=5)
-    ap.add_argument("--variant", type=int, default=0, help="launch variant of the fused kernel (tuning aid)")
+    ap.add_argument("--variant", type=int, default=-1, help="launch variant of the fused kernel (tuning aid)")
     ap.add_argument("--rows", type=int, default=0, help="rows per block of the fused kernel (0 = automatic)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--traffic", type=float, default=None,

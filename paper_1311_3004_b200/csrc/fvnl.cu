@@ -9,7 +9,7 @@
 #include <vector>
 
 #include "../../include/fvnl.h"
-#include "fvnl_fused.cuh"
+#include "fvnl_pipe.cuh"
 
 using namespace fvnl;
 
@@ -129,7 +129,8 @@ struct fvnl_ctx {
 };
 
 static const size_t MAX_SPANS = 1 << 16;
-static const int N_FUSED_VARIANTS = 4;     // launch variants of the fused kernel (launch_fused)
+static const int N_FUSED_VARIANTS = 8;
+static const int DEFAULT_VARIANT = 4;       // k_step_pipe<128, 2>     // launch variants of the fused kernel (launch_fused)
 
 // Event pair around one kernel launch (timing on only).
 struct SpanGuard {
@@ -226,6 +227,7 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
     c->have_state = true;
     c->need_prepass = true;
     c->kernel = FVNL_KERNEL_DEFAULT;
+    c->variant = DEFAULT_VARIANT;
     if (!ok) { (void)cudaGetLastError(); fvnl_destroy(c); return FVNL_ECUDA; }
     *out = c;
     return FVNL_OK;
@@ -330,7 +332,7 @@ static const FusedVariant FUSED_VARIANTS[] = {{128, 3}, {256, 2}, {128, 4}, {256
 // number of chunks that maximises  (work in full waves) x (useful rows per marched row):
 //     efficiency = blocks / (ceil(blocks / slots) * slots)  *  rows / (rows + 7)
 // (7 = the pipeline fill of a chunk: 3 halo rows below, 3 above, 1 for the y-sweep running one row behind).
-static int fused_rows(const fvnl_ctx* c, int strips, int slots) {
+static int fused_rows(const fvnl_ctx* c, int strips, int slots, int fill = 7) {
     const int ny = c->g.ny;
     if (c->rows_per_block > 0) return c->rows_per_block < ny ? c->rows_per_block : ny;
     int best_rows = ny;
@@ -341,7 +343,7 @@ static int fused_rows(const fvnl_ctx* c, int strips, int slots) {
         const int nch = (ny + rows - 1) / rows;
         const long blocks = (long)strips * nch;
         const long waves = (blocks + slots - 1) / slots;
-        const double eff = (double)blocks / (double)(waves * slots) * rows / (rows + 7.0);
+        const double eff = (double)blocks / (double)(waves * slots) * rows / (rows + (double)fill);
         if (eff > best + 1e-9) { best = eff; best_rows = rows; }
     }
     return best_rows;
@@ -362,8 +364,27 @@ static void launch_fused_t(fvnl_ctx* c, double** a, double** b) {
     k_step_fused<BX, MINB><<<grd, BX, fused_smem_bytes<BX>(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
 }
 
+template <int BX, int MINB>
+static void launch_pipe_t(fvnl_ctx* c, double** a, double** b) {
+    const Grid& g = c->g;
+    const int strips = (g.nx + (BX - 6) - 1) / (BX - 6);
+    const int rows = fused_rows(c, strips, 148 * MINB, 10);
+    const dim3 grd(strips, (g.ny + rows - 1) / rows);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_step_pipe<BX, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, pipe_smem_bytes<BX>());
+        attr_set = true;
+    }
+    SpanGuard sp(c, FVNL_TIMED_STEP);
+    k_step_pipe<BX, MINB><<<grd, BX, pipe_smem_bytes<BX>(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
+}
+
 static void launch_fused(fvnl_ctx* c, double** a, double** b) {
     switch (c->variant) {
+        case 4: launch_pipe_t<128, 2>(c, a, b); break;
+        case 5: launch_pipe_t<128, 3>(c, a, b); break;
+        case 6: launch_pipe_t<256, 1>(c, a, b); break;
+        case 7: launch_pipe_t<160, 2>(c, a, b); break;
         case 1: launch_fused_t<160, 3>(c, a, b); break;
         case 2: launch_fused_t<96, 5>(c, a, b); break;
         case 3: launch_fused_t<64, 7>(c, a, b); break;
