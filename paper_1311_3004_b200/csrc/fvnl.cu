@@ -10,6 +10,7 @@
 
 #include "../../include/fvnl.h"
 #include "fvnl_pipe.cuh"
+#include "fvnl_ws.cuh"
 
 using namespace fvnl;
 
@@ -129,8 +130,8 @@ struct fvnl_ctx {
 };
 
 static const size_t MAX_SPANS = 1 << 16;
-static const int N_FUSED_VARIANTS = 8;
-static const int DEFAULT_VARIANT = 4;       // k_step_pipe<128, 2>     // launch variants of the fused kernel (launch_fused)
+static const int N_FUSED_VARIANTS = 12;
+static const int DEFAULT_VARIANT = 0;       // k_step_fused<128, 3>     // launch variants of the fused kernel (launch_fused)
 
 // Event pair around one kernel launch (timing on only).
 struct SpanGuard {
@@ -325,8 +326,6 @@ static int ensure_star(fvnl_ctx* c) {
 
 // Fused step: strips of BX columns (BX - 6 produce output) x chunks of `rows` rows.  Launch variants
 // (FVNL_OPT_VARIANT): block width and the register budget the compiler was given (blocks per SM).
-struct FusedVariant { int bx, minb; };
-static const FusedVariant FUSED_VARIANTS[] = {{128, 3}, {256, 2}, {128, 4}, {256, 1}};
 
 // Rows per chunk.  All blocks do the same work, so the grid runs as "waves" of `slots` resident blocks: pick the
 // number of chunks that maximises  (work in full waves) x (useful rows per marched row):
@@ -379,8 +378,32 @@ static void launch_pipe_t(fvnl_ctx* c, double** a, double** b) {
     k_step_pipe<BX, MINB><<<grd, BX, pipe_smem_bytes<BX>(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
 }
 
+template <int XREGS, int YREGS>
+static void launch_ws_t(fvnl_ctx* c, double** a, double** b) {
+    const Grid& g = c->g;
+    const int strips = (g.nx + (WS_COLS - 6) - 1) / (WS_COLS - 6);
+    const int per_sm = 65536 / (128 * (XREGS + YREGS));
+    const int rows = fused_rows(c, strips, 148 * per_sm, 7);
+    const dim3 grd(strips, (g.ny + rows - 1) / rows);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_step_ws<XREGS, YREGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, ws_smem_bytes());
+        attr_set = true;
+    }
+    SpanGuard sp(c, FVNL_TIMED_STEP);
+    k_step_ws<XREGS, YREGS><<<grd, 256, ws_smem_bytes(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
+}
+
 static void launch_fused(fvnl_ctx* c, double** a, double** b) {
-    switch (c->variant) {
+    int variant = c->variant;
+    if (variant >= 8) {                     // the warp-specialised kernel has no analytic-source code (fvnl_ws.cuh)
+        for (int s = 0; s < 4; ++s)
+            if (c->g.side[s].kind == BC_SOURCE) variant = 0;
+    }
+    switch (variant) {
+        case 8: launch_ws_t<128, 128>(c, a, b); break;
+        case 9: launch_ws_t<96, 160>(c, a, b); break;
+        case 11: launch_ws_t<168, 168>(c, a, b); break;
         case 4: launch_pipe_t<128, 2>(c, a, b); break;
         case 5: launch_pipe_t<128, 3>(c, a, b); break;
         case 6: launch_pipe_t<256, 1>(c, a, b); break;

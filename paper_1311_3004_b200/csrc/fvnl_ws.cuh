@@ -1,0 +1,310 @@
+// fvnl_ws.cuh -- the one-pass step kernel, warp specialised: half of a block's warps run the x-sweep, the other half
+// the y-sweep and the source step, on the same strip of columns.
+//
+// Why.  The fused kernel (fvnl_fused.cuh) carries the whole rolling state of a column in one thread: ~168 registers,
+// 12 warps per SM, and since a warp issues in order and a dependent FP64 operation waits 9 cycles (measured), the
+// FP64 pipe sits half idle (profiles/).  The x-sweep of a row needs NO state from earlier rows; the y-sweep needs the
+// rolling window.  Splitting the two gives x-warps a small register footprint and y-warps a medium one
+// (setmaxnreg moves registers from the first to the second), 16 warps per SM instead of 12, and two independent
+// instruction streams per scheduler that never wait on each other's barriers except once per tick:
+//     tick r, X warps :  Q^n(., r) -> cells -> [bar X] -> Riemann solves -> [bar X] -> limited fluxes
+//                        -> publish  u = Q^n - lam_x G+  and  G-  of row r (parity r&1)            -> [bar ALL]
+//     tick r, Y warps :  Q*(., r-1) = u - lam_x G-(right neighbour)  (published in tick r-1)
+//                        -> y-Riemann solve, limited y-flux -> Q**(., r-3) -> source step -> Q^{n+1}(., r-4) -> HBM
+//                        -> publish z of Q** for the neighbours' source step (parity r&1)        -> [bar ALL]
+// Arithmetic, ghost rules and validity masks are those of fvnl_fused.cuh.
+//
+// This kernel serves grids WITHOUT an analytic SOURCE edge (periodic / extrapolation / reflecting): ptxas 12.9 crashes
+// on setmaxnreg in a kernel that also calls the out-of-line source functions (sin / exp / tanh slow paths), and the
+// source cells sit in one strip only anyway.  fvnl_step launches k_step_fused when any edge is a SOURCE.
+#pragma once
+#include "fvnl_fused.cuh"
+
+namespace fvnl {
+
+constexpr int WS_COLS = 128;                  // columns of a strip = threads of each group
+// shared memory (bytes): arrays of double2, WS_COLS + 2 elements each
+//   single-buffered (X group only):   0 (q1,q2)  1 (q3,hz2)  2 (hz3,-)  3 (al1,s1)  4 (r31,al3)  5 (al2,s2)  6 (r32,-)
+//   double-buffered by tick parity:   7 (m1,m2)  8 (m3,-)  9 (u1,u2)  10 (u3,-)  [X -> Y]     11 (z2,z3)  [Y -> Y]
+__host__ __device__ constexpr int ws_arr(int k) { return k * (WS_COLS + 2) * 16; }
+__host__ __device__ constexpr int ws_arr2(int k, int parity) { return ws_arr(7 + 2 * (k - 7) + parity); }
+__host__ __device__ constexpr int ws_ring_off() { return ws_arr(7 + 2 * 5); }
+__host__ __device__ constexpr int ws_smem_bytes() { return ws_ring_off() + 4 * 3 * WS_COLS * 8; }
+
+__device__ __forceinline__ void bar_x() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+__device__ __forceinline__ void bar_all() { asm volatile("bar.sync 2, 256;" ::: "memory"); }
+
+struct XThread {
+    ColMap cm;
+    int i, special;
+    char *p, *pq;
+    double smx;
+    int mqx, mdx;
+};
+
+// One tick of an X warp: the x-sweep of row r up to the two halves of the update (27).
+template <int P, bool STEADY>
+__device__ __forceinline__ void ws_xtick(const Grid& g, const StepK& k, XThread& th, int r,
+                                         const double* __restrict__ q1, const double* __restrict__ q2,
+                                         const double* __restrict__ q3) {
+    char* const p = th.p;
+    RowMap rm, rm_pre;                                                        // rows r and r+2 (the one to prefetch)
+    if (STEADY) {
+        rm.row = r; rm.neg3 = false; rm.ysrc = -1;
+        rm_pre.row = r + 2;
+    } else {
+        rm = map_row(g, r);
+        rm_pre = map_row(g, r + 2);
+    }
+    cp_async_wait<1>();                                                       // row r has landed
+    double a1, a2, a3;
+    {
+        const char* ps = th.pq + (r & 3) * (3 * WS_COLS * 8);
+        a1 = lds1(ps); a2 = lds1(ps + WS_COLS * 8); a3 = lds1(ps + 2 * WS_COLS * 8);
+        char* pd = th.pq + ((r + 2) & 3) * (3 * WS_COLS * 8);
+        const size_t idx = (size_t)rm_pre.row * g.nx + th.cm.col;
+        cp_async8(pd, q1 + idx); cp_async8(pd + WS_COLS * 8, q2 + idx); cp_async8(pd + 2 * WS_COLS * 8, q3 + idx);
+        cp_async_commit();
+    }
+    if ((th.special & 4) || (!STEADY && rm.neg3)) {                           // ghost column / row of a REFLECT side: rare
+        if (!STEADY && rm.neg3) a3 = -a3;
+        if (th.special & 4) a2 = -a2;
+    }
+    int tq = 0x7fffffff, td = 0x7fffffff;
+    const Cx cx = cell_of(a1, a2, a3, tq);
+    sts2(p + ws_arr(0), cx.q1, cx.q2); sts2(p + ws_arr(1), cx.q3, cx.hz2); sts1(p + ws_arr(2), cx.hz3);
+    bar_x();                                                                  // cells visible
+    Cx L;
+    {
+        const double2 u0 = lds2(p + ws_arr(0) - 16), u1 = lds2(p + ws_arr(1) - 16);
+        L.q1 = u0.x; L.q2 = u0.y; L.q3 = u1.x; L.hz2 = u1.y; L.hz3 = lds1(p + ws_arr(2) - 16);
+    }
+    const Wv w = riemann2(L, cx, k.b2, k.omb2, td);
+    const double rn1 = rnorm(w.s1, w.r31), rn2 = rnorm(w.s2, w.r32);
+    sts2(p + ws_arr(3), w.al1, w.s1); sts2(p + ws_arr(4), w.r31, w.al3); sts2(p + ws_arr(5), w.al2, w.s2);
+    sts1(p + ws_arr(6), w.r32);
+    if (STEADY || (unsigned)r < (unsigned)g.ny) {
+        th.mqx = min(th.mqx, tq); th.mdx = min(th.mdx, td);
+        th.smx = dmax(th.smx, fabs(hi_word(w.v) < 0 ? w.s2 : w.s1));          // max(|s1|,|s2|) = |v| + a
+    }
+    bar_x();                                                                  // waves visible
+    {
+        const char* u1 = p + (hi_word(w.s1) < 0 ? 16 : -16);                  // upwind interface
+        const char* u2 = p + (hi_word(w.s2) < 0 ? 16 : -16);
+        const char* u3 = p + (hi_word(w.v) < 0 ? 16 : -16);
+        const double2 k1 = lds2(u1 + ws_arr(3)), k2 = lds2(u2 + ws_arr(5));
+        const double k1r = lds1(u1 + ws_arr(4)), k2r = lds1(u2 + ws_arr(6)), k3 = lds1(u3 + ws_arr(4) + 8);
+        const double b1 = k1.x * rdot(k1.y, k1r, w.s1, w.r31) * rn1;
+        const double b2 = k2.x * rdot(k2.y, k2r, w.s2, w.r32) * rn2;
+        const Fl F = flux2(w, b1, b2, k3, k.lamx);
+        // the two halves of (27) for row r: what this interface sends left, and this column's own part
+        sts2(p + ws_arr2(7, P), F.m1, F.m2); sts1(p + ws_arr2(8, P), F.m3);
+        sts2(p + ws_arr2(9, P), fma(-k.lamx, F.p1, a1), fma(-k.lamx, F.p2, a2));
+        sts1(p + ws_arr2(10, P), fma(-k.lamx, F.p3, a3));
+    }
+    bar_all();                                                                // row r handed to the Y warps
+}
+
+// z of the one-deep ghost of Q** at a non-periodic, non-source edge: EXTRAP copies, REFLECT negates the normal velocity.
+__device__ __forceinline__ double2 ghost_z_plain(const Grid& g, int sd, double z2, double z3) {
+    if (g.side[sd].kind == BC_REFLECT) return sd < 2 ? make_double2(-z2, z3) : make_double2(z2, -z3);
+    return make_double2(z2, z3);
+}
+
+struct YThread {
+    int i, special;
+    bool out_col;
+    char* p;
+    double smy;
+    int mqy, mdy, mxo;
+};
+
+struct YCarry {
+    double gp1, gp2, gp3;                    // right-going part of the y-interface below the newest one, y-form
+    double c1, c2, c3, zC2, zC3;             // Q**(ry-3) and its z
+    double zS2, zS3;                         // z of Q**(ry-4)
+};
+
+// One tick of a Y warp (tick r works on ry = r-1): Q*(., ry) from what the X warps published in the previous tick,
+// y-interface ry-1/2 (N), limited flux of interface ry-3/2 (A), Q**(., ry-2), source step for row ry-3.
+// P = r & 1: parity this tick publishes into; it reads parity P^1.
+template <int P, bool STEADY>
+__device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread& th, YCarry& cy, YSet& Y0, YSet& Y1, int r,
+                                         double* __restrict__ o1, double* __restrict__ o2, double* __restrict__ o3) {
+    YSet& N = P ? Y1 : Y0;
+    const YSet& A = P ? Y0 : Y1;
+    constexpr int R = P ^ 1;
+    char* const p = th.p;
+    const int ry = r - 1;
+    double s1, s2, s3;                                                        // Q*(i, ry): the update (27) completed
+    {
+        const double2 u = lds2(p + ws_arr2(9, R)), gm = lds2(p + ws_arr2(7, R) + 16);
+        const double u3 = lds1(p + ws_arr2(10, R)), gm3 = lds1(p + ws_arr2(8, R) + 16);
+        s1 = fma(-k.lamx, gm.x, u.x); s2 = fma(-k.lamx, gm.y, u.y); s3 = fma(-k.lamx, gm3, u3);
+    }
+    double2 zW = lds2(p + ws_arr2(11, R) - 16), zE = lds2(p + ws_arr2(11, R) + 16);   // z of row ry-3, published last tick
+    const double b1o = N.c.q1, b2o = N.c.q2, b3o = N.c.q3;                    // Q*(ry-2), y-form (before N is overwritten)
+    int tqy = 0x7fffffff, tdy = 0x7fffffff;
+    N.c = cell_of(s1, s3, s2, tqy);                                           // positions 2,3 switched
+    N.w = riemann2(A.c, N.c, k.b2, k.omb2, tdy);
+    N.rn1 = rnorm(N.w.s1, N.w.r31); N.rn2 = rnorm(N.w.s2, N.w.r32);
+    const double d1 = rdot(A.w.s1, A.w.r31, N.w.s1, N.w.r31), d2 = rdot(A.w.s2, A.w.r32, N.w.s2, N.w.r32);
+    N.pb1 = A.w.al1 * d1 * N.rn1; N.pb2 = A.w.al2 * d2 * N.rn2; N.pb3 = A.w.al3;      // if A is N's upwind side
+    const double hb1 = N.w.al1 * d1 * A.rn1, hb2 = N.w.al2 * d2 * A.rn2;              // if N is A's upwind side
+    const Fl G = flux2(A.w, hi_word(A.w.s1) < 0 ? hb1 : A.pb1, hi_word(A.w.s2) < 0 ? hb2 : A.pb2,
+                       hi_word(A.w.v) < 0 ? N.w.al3 : A.pb3, k.lamy);
+    const double n1 = fma(-k.lamy, cy.gp1 + G.m1, b1o);                       // Q**(i, ry-2); physical order n1, n2, n3
+    const double n3 = fma(-k.lamy, cy.gp2 + G.m2, b2o);
+    const double n2 = fma(-k.lamy, cy.gp3 + G.m3, b3o);
+    cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3;
+    if (STEADY || (unsigned)(ry - k.ylo) <= (unsigned)k.ycnt) {               // y-interface ry-1/2 is one the scheme solves
+        th.mqy = min(th.mqy, tqy); th.mdy = min(th.mdy, tdy);
+        if (STEADY || (unsigned)ry <= (unsigned)g.ny) th.smy = dmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
+    }
+    // ---- source step (26): x part of row ry-3, publish z of row ry-2, finish row ry-3 -------------------------------
+    if (th.special & 3) {
+        if (th.special & 1) zW = ghost_z_plain(g, SIDE_XLO, cy.zC2, cy.zC3);
+        if (th.special & 2) zE = ghost_z_plain(g, SIDE_XHI, cy.zC2, cy.zC3);
+    }
+    const double H2 = fma(k.k2, cy.zC2, fma(k.kapx, zE.x + zW.x, cy.c2));
+    const double H3 = fma(k.k2, cy.zC3, fma(k.kapx, zE.y + zW.y, cy.c3));
+    const double rq = rcp_o1(n1);
+    const double zN2 = n2 * rq, zN3 = n3 * rq;
+    sts2(p + ws_arr2(11, P), zN2, zN3);
+    const int Ro = ry - 3;
+    if (STEADY || Ro >= k.j0) {                                               // Ro < j1 by the loop bound
+        double y2 = zN2 + cy.zS2, y3 = zN3 + cy.zS3;
+        if (!STEADY && !k.py && (Ro == 0 || Ro == g.ny - 1)) {
+            double2 lo = make_double2(cy.zS2, cy.zS3), hi = make_double2(zN2, zN3);
+            if (Ro == 0) lo = ghost_z_plain(g, SIDE_YLO, cy.zC2, cy.zC3);
+            if (Ro == g.ny - 1) hi = ghost_z_plain(g, SIDE_YHI, cy.zC2, cy.zC3);
+            y2 = hi.x + lo.x; y3 = hi.y + lo.y;
+        }
+        const double w2 = fma(k.kapy, y2, H2), w3 = fma(k.kapy, y3, H3);
+        if (th.out_col) {
+            const size_t o = (size_t)Ro * g.nx + th.i;
+            o1[o] = cy.c1; o2[o] = w2; o3[o] = w3;
+            th.mxo = max(th.mxo, max(hi_word(cy.c1) & 0x7fffffff, max(hi_word(w2) & 0x7fffffff, hi_word(w3) & 0x7fffffff)));
+        }
+    }
+    cy.zS2 = cy.zC2; cy.zS3 = cy.zC3;
+    cy.c1 = n1; cy.c2 = n2; cy.c3 = n3; cy.zC2 = zN2; cy.zC3 = zN3;
+    bar_all();
+}
+
+// The step kernel.  grid = (strips, chunks); block = 256 threads (warps 0-3: X group, warps 4-7: Y group);
+// dynamic shared memory = ws_smem_bytes().  XREGS / YREGS: register budgets of the two groups (setmaxnreg); the
+// kernel is launched with their mean.
+template <int XREGS, int YREGS>
+__global__ void __launch_bounds__(256, 65536 / (128 * (XREGS + YREGS)))
+k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __restrict__ q2,
+          const double* __restrict__ q3, double* __restrict__ o1, double* __restrict__ o2, double* __restrict__ o3,
+          int rows) {
+    extern __shared__ __align__(16) char smem[];
+    const int tid = threadIdx.x;
+    for (int j = tid; j < ws_smem_bytes() / 8; j += 256) reinterpret_cast<double*>(smem)[j] = 1.0;   // finite fill
+
+    StepK k;
+    k.t = clk->t; k.lamx = clk->lamx; k.lamy = clk->lamy; k.kapx = clk->kapx; k.kapy = clk->kapy;
+    k.k2 = -2.0 * (k.kapx + k.kapy);
+    k.b2 = 2.0 * (g.beta - 1.0); k.omb2 = 1.0 - k.b2;
+    k.j0 = (int)blockIdx.y * rows; k.j1 = min(k.j0 + rows, g.ny);
+    k.ylo = max(k.j0 - 2, -1); k.ycnt = g.ny + 1 - k.ylo;
+    k.px = g.side[SIDE_XLO].kind == BC_PERIODIC; k.py = g.side[SIDE_YLO].kind == BC_PERIODIC;
+    k.any_src = false; k.any_refl = false;
+    const int c = tid & (WS_COLS - 1);                             // column of the strip
+    const int i = (int)blockIdx.x * (WS_COLS - 6) - 3 + c;         // column on the ghost-extended mesh
+    const int r0 = k.j0 - 3, rend = k.j1 + 4;                      // the Y group runs one row behind, output row = r - 4
+    double smx = 0.0, smy = 0.0;
+    int flags = 0;
+    __syncthreads();                                               // (the fill above is complete)
+
+    if (tid < WS_COLS) {
+        // ================================= X group: the x-sweep =======================================================
+        if constexpr (XREGS == 96) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
+        if constexpr (XREGS == 104) asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
+        if constexpr (XREGS == 88) asm volatile("setmaxnreg.dec.sync.aligned.u32 88;");
+        XThread th;
+        th.i = i;
+        th.cm = map_column(g, i);
+        th.special = (th.cm.neg2 ? 4 : 0) | (th.cm.xsrc >= 0 ? 8 : 0);
+        th.p = smem + (c + 1) * 16;
+        th.pq = smem + ws_ring_off() + c * 8;
+        th.smx = 0.0; th.mqx = th.mdx = 0x7fffffff;
+        for (int d = 0; d < 2; ++d) {                              // rows r0 and r0+1 start their way into the ring
+            const RowMap rm = map_row(g, r0 + d);
+            const size_t idx = (size_t)rm.row * g.nx + th.cm.col;
+            char* pd = th.pq + ((r0 + d) & 3) * (3 * WS_COLS * 8);
+            cp_async8(pd, q1 + idx); cp_async8(pd + WS_COLS * 8, q2 + idx); cp_async8(pd + 2 * WS_COLS * 8, q3 + idx);
+            cp_async_commit();
+        }
+        int r = r0;
+        const int slo = 0, shi = min(rend - 1, g.ny - 3);          // steady: rows r .. r+2 are interior rows
+        while (r < rend && (r < slo || (r & 1))) {
+            if (r & 1) ws_xtick<1, false>(g, k, th, r, q1, q2, q3); else ws_xtick<0, false>(g, k, th, r, q1, q2, q3);
+            ++r;
+        }
+        for (; r + 1 <= shi; r += 2) {
+            ws_xtick<0, true>(g, k, th, r, q1, q2, q3);
+            ws_xtick<1, true>(g, k, th, r + 1, q1, q2, q3);
+        }
+        while (r < rend) {
+            if (r & 1) ws_xtick<1, false>(g, k, th, r, q1, q2, q3); else ws_xtick<0, false>(g, k, th, r, q1, q2, q3);
+            ++r;
+        }
+        cp_async_wait<0>();
+        const bool x_if_m = c >= 1 && i >= 0 && i <= g.nx;          // x-interface i-1/2 touches an interior cell
+        const bool x_if_f = c >= 1 && i >= -1 && i <= g.nx + 1;     // ... is one the scheme solves
+        const bool x_cell = i >= -2 && i <= g.nx + 1;
+        if (x_cell && th.mqx <= 0) flags |= F_ENONPOS;
+        if (x_if_f && th.mdx < 0) flags |= F_ENONREAL;
+        if (x_if_m) smx = th.smx;
+    } else {
+        // ================================= Y group: the y-sweep and the source step ===================================
+        if constexpr (YREGS == 160) asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
+        if constexpr (YREGS == 152) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
+        if constexpr (YREGS == 168) asm volatile("setmaxnreg.inc.sync.aligned.u32 168;");
+        YThread th;
+        th.i = i;
+        th.special = (!k.px && i == 0 ? 1 : 0) | (!k.px && i == g.nx - 1 ? 2 : 0);
+        th.out_col = c >= 3 && c <= WS_COLS - 4 && i >= 0 && i < g.nx;
+        th.p = smem + (c + 1) * 16;
+        th.smy = 0.0; th.mqy = th.mdy = 0x7fffffff; th.mxo = 0;
+        YSet Y0, Y1;
+        Y0.c = {1.0, 0.0, 0.0, 0.0, 0.0};
+        Y0.w = {0.0, 1.0, 0.0, 0.0, -1.0, 0.0, 0.0, 0.0};
+        Y0.rn1 = Y0.rn2 = 0.5; Y0.pb1 = Y0.pb2 = Y0.pb3 = 0.0;
+        Y1 = Y0;
+        YCarry cy;
+        cy.gp1 = cy.gp2 = cy.gp3 = 0.0;
+        cy.c1 = 1.0; cy.c2 = cy.c3 = cy.zC2 = cy.zC3 = cy.zS2 = cy.zS3 = 0.0;
+        int r = r0;
+        // steady: interface ry-1/2 (ry = r-1) is a real one, output row r-4 >= j0 and away from the y edges
+        const int slo = max(k.j0 + 4, k.py ? 0 : 5), shi = min(rend - 1, g.ny);
+        while (r < rend && (r < slo || (r & 1))) {
+            if (r & 1) ws_ytick<1, false>(g, k, th, cy, Y0, Y1, r, o1, o2, o3); else ws_ytick<0, false>(g, k, th, cy, Y0, Y1, r, o1, o2, o3);
+            ++r;
+        }
+        for (; r + 1 <= shi; r += 2) {
+            ws_ytick<0, true>(g, k, th, cy, Y0, Y1, r, o1, o2, o3);
+            ws_ytick<1, true>(g, k, th, cy, Y0, Y1, r + 1, o1, o2, o3);
+        }
+        while (r < rend) {
+            if (r & 1) ws_ytick<1, false>(g, k, th, cy, Y0, Y1, r, o1, o2, o3); else ws_ytick<0, false>(g, k, th, cy, Y0, Y1, r, o1, o2, o3);
+            ++r;
+        }
+        const bool y_col = c >= 2 && c <= WS_COLS - 3 && i >= 0 && i < g.nx;
+        if (y_col && th.mqy <= 0) flags |= F_ENONPOS;
+        if (y_col && th.mdy < 0) flags |= F_ENONREAL;
+        if (th.mxo >= 0x7ff00000) flags |= F_ENAN;
+        if (y_col) smy = th.smy;
+    }
+    // ---- reductions: M of and the sticky flags ---------------------------------------------------------
+    __syncthreads();
+    block_max_to(&clk->sx_bits, smx);
+    __syncthreads();
+    block_max_to(&clk->sy_bits, smy);
+    block_flags_to(&clk->flags, flags);
+}
+
+}  // namespace fvnl
