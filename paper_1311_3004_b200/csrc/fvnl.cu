@@ -383,7 +383,7 @@ static void launch_ws_t(fvnl_ctx* c, double** a, double** b) {
     const Grid& g = c->g;
     const int strips = (g.nx + (WS_COLS - 6) - 1) / (WS_COLS - 6);
     const int per_sm = 65536 / (128 * (XREGS + YREGS));
-    const int rows = fused_rows(c, strips, 148 * per_sm, 7);
+    const int rows = fused_rows(c, strips, 148 * per_sm, 8);
     const dim3 grd(strips, (g.ny + rows - 1) / rows);
     static bool attr_set = false;
     if (!attr_set) {

@@ -121,47 +121,34 @@ struct YThread {
 
 struct YCarry {
     double gp1, gp2, gp3;                    // right-going part of the y-interface below the newest one, y-form
-    double c1, c2, c3, zC2, zC3;             // Q**(ry-3) and its z
-    double zS2, zS3;                         // z of Q**(ry-4)
+    double q1, q2, q3;                       // Q*(., ry-3), y-form
+    double c1, c2, c3, zC2, zC3;             // Q**(ry-4) and its z
+    double zS2, zS3;                         // z of Q**(ry-5)
 };
 
-// One tick of a Y warp (tick r works on ry = r-1): Q*(., ry) from what the X warps published in the previous tick,
-// y-interface ry-1/2 (N), limited flux of interface ry-3/2 (A), Q**(., ry-2), source step for row ry-3.
-// P = r & 1: parity this tick publishes into; it reads parity P^1.
+// One tick of a Y warp (tick r works on ry = r-1).  Two independent chains, so that the warp has two instructions to
+// choose from at every step:
+//   chain 1:  Q*(., ry) from what the X warps published in the previous tick -> cell -> y-Riemann solve at ry-1/2 (N)
+//             -> limiter inputs between N and the interface below it (A), which are now final for A;
+//   chain 2:  limited flux of the interface two below N (B, at ry-5/2: its limiter inputs became final in the previous
+//             tick) -> Q**(., ry-3) -> source step for row ry-4 -> Q^{n+1}(., ry-4) -> HBM.
+// P = r & 1: parity this tick publishes into (it reads parity P^1); Y[P] holds B on entry and N on exit, Y[P^1] is A.
 template <int P, bool STEADY>
 __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread& th, YCarry& cy, YSet& Y0, YSet& Y1, int r,
                                          double* __restrict__ o1, double* __restrict__ o2, double* __restrict__ o3) {
     YSet& N = P ? Y1 : Y0;
-    const YSet& A = P ? Y0 : Y1;
+    YSet& A = P ? Y0 : Y1;
     constexpr int R = P ^ 1;
     char* const p = th.p;
     const int ry = r - 1;
-    double s1, s2, s3;                                                        // Q*(i, ry): the update (27) completed
-    {
-        const double2 u = lds2(p + ws_arr2(9, R)), gm = lds2(p + ws_arr2(7, R) + 16);
-        const double u3 = lds1(p + ws_arr2(10, R)), gm3 = lds1(p + ws_arr2(8, R) + 16);
-        s1 = fma(-k.lamx, gm.x, u.x); s2 = fma(-k.lamx, gm.y, u.y); s3 = fma(-k.lamx, gm3, u3);
-    }
-    double2 zW = lds2(p + ws_arr2(11, R) - 16), zE = lds2(p + ws_arr2(11, R) + 16);   // z of row ry-3, published last tick
-    const double b1o = N.c.q1, b2o = N.c.q2, b3o = N.c.q3;                    // Q*(ry-2), y-form (before N is overwritten)
-    int tqy = 0x7fffffff, tdy = 0x7fffffff;
-    N.c = cell_of(s1, s3, s2, tqy);                                           // positions 2,3 switched, PAPER.md:155,271
-    N.w = riemann2(A.c, N.c, k.b2, k.omb2, tdy);
-    N.rn1 = rnorm(N.w.s1, N.w.r31); N.rn2 = rnorm(N.w.s2, N.w.r32);
-    const double d1 = rdot(A.w.s1, A.w.r31, N.w.s1, N.w.r31), d2 = rdot(A.w.s2, A.w.r32, N.w.s2, N.w.r32);
-    N.pb1 = A.w.al1 * d1 * N.rn1; N.pb2 = A.w.al2 * d2 * N.rn2; N.pb3 = A.w.al3;      // if A is N's upwind side
-    const double hb1 = N.w.al1 * d1 * A.rn1, hb2 = N.w.al2 * d2 * A.rn2;              // if N is A's upwind side
-    const Fl G = flux2(A.w, hi_word(A.w.s1) < 0 ? hb1 : A.pb1, hi_word(A.w.s2) < 0 ? hb2 : A.pb2,
-                       hi_word(A.w.v) < 0 ? N.w.al3 : A.pb3, k.lamy);
-    const double n1 = fma(-k.lamy, cy.gp1 + G.m1, b1o);                       // Q**(i, ry-2); physical order n1, n2, n3
-    const double n3 = fma(-k.lamy, cy.gp2 + G.m2, b2o);
-    const double n2 = fma(-k.lamy, cy.gp3 + G.m3, b3o);
+    // ---- chain 2: flux of B, Q**(., ry-3), source step ----------------------------------------------------------------
+    const Fl G = flux2(N.w, N.pb1, N.pb2, N.pb3, k.lamy);                     // N still holds B
+    const double n1 = fma(-k.lamy, cy.gp1 + G.m1, cy.q1);                     // Q**(i, ry-3); physical order n1, n2, n3
+    const double n3 = fma(-k.lamy, cy.gp2 + G.m2, cy.q2);
+    const double n2 = fma(-k.lamy, cy.gp3 + G.m3, cy.q3);
     cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3;
-    if (STEADY || (unsigned)(ry - k.ylo) <= (unsigned)k.ycnt) {               // y-interface ry-1/2 is one the scheme solves
-        th.mqy = min(th.mqy, tqy); th.mdy = min(th.mdy, tdy);
-        if (STEADY || (unsigned)ry <= (unsigned)g.ny) th.smy = dmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
-    }
-    // ---- source step (26): x part of row ry-3, publish z of row ry-2, finish row ry-3 -------------------------------
+    cy.q1 = N.c.q1; cy.q2 = N.c.q2; cy.q3 = N.c.q3;                           // Q*(ry-2), y-form: next tick's lower row
+    double2 zW = lds2(p + ws_arr2(11, R) - 16), zE = lds2(p + ws_arr2(11, R) + 16);   // z of row ry-4, published last tick
     if (th.special & 3) {
         if (th.special & 1) zW = ghost_z_plain(g, SIDE_XLO, cy.zC2, cy.zC3);
         if (th.special & 2) zE = ghost_z_plain(g, SIDE_XHI, cy.zC2, cy.zC3);
@@ -171,7 +158,7 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
     const double rq = rcp_o1(n1);
     const double zN2 = n2 * rq, zN3 = n3 * rq;
     sts2(p + ws_arr2(11, P), zN2, zN3);
-    const int Ro = ry - 3;
+    const int Ro = ry - 4;
     if (STEADY || Ro >= k.j0) {                                               // Ro < j1 by the loop bound
         double y2 = zN2 + cy.zS2, y3 = zN3 + cy.zS3;
         if (!STEADY && !k.py && (Ro == 0 || Ro == g.ny - 1)) {
@@ -189,6 +176,28 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
     }
     cy.zS2 = cy.zC2; cy.zS3 = cy.zC3;
     cy.c1 = n1; cy.c2 = n2; cy.c3 = n3; cy.zC2 = zN2; cy.zC3 = zN3;
+
+    // ---- chain 1: Q*(., ry), interface ry-1/2 (N), final limiter inputs of A ---------------------------------------------
+    double s1, s2, s3;                                                        // Q*(i, ry): the update (27) completed
+    {
+        const double2 u = lds2(p + ws_arr2(9, R)), gm = lds2(p + ws_arr2(7, R) + 16);
+        const double u3 = lds1(p + ws_arr2(10, R)), gm3 = lds1(p + ws_arr2(8, R) + 16);
+        s1 = fma(-k.lamx, gm.x, u.x); s2 = fma(-k.lamx, gm.y, u.y); s3 = fma(-k.lamx, gm3, u3);
+    }
+    int tqy = 0x7fffffff, tdy = 0x7fffffff;
+    N.c = cell_of(s1, s3, s2, tqy);                                           // positions 2,3 switched, PAPER.md:155,271
+    N.w = riemann2(A.c, N.c, k.b2, k.omb2, tdy);
+    N.rn1 = rnorm(N.w.s1, N.w.r31); N.rn2 = rnorm(N.w.s2, N.w.r32);
+    const double d1 = rdot(A.w.s1, A.w.r31, N.w.s1, N.w.r31), d2 = rdot(A.w.s2, A.w.r32, N.w.s2, N.w.r32);
+    N.pb1 = A.w.al1 * d1 * N.rn1; N.pb2 = A.w.al2 * d2 * N.rn2; N.pb3 = A.w.al3;      // if A is N's upwind side
+    const double hb1 = N.w.al1 * d1 * A.rn1, hb2 = N.w.al2 * d2 * A.rn2;              // if N is A's upwind side
+    A.pb1 = hi_word(A.w.s1) < 0 ? hb1 : A.pb1;                                // A's upwind side is now known
+    A.pb2 = hi_word(A.w.s2) < 0 ? hb2 : A.pb2;
+    A.pb3 = hi_word(A.w.v) < 0 ? N.w.al3 : A.pb3;
+    if (STEADY || (unsigned)(ry - k.ylo) <= (unsigned)k.ycnt) {               // y-interface ry-1/2 is one the scheme solves
+        th.mqy = min(th.mqy, tqy); th.mdy = min(th.mdy, tdy);
+        if (STEADY || (unsigned)ry <= (unsigned)g.ny) th.smy = dmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
+    }
     bar_all();
 }
 
@@ -214,7 +223,7 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
     k.any_src = false; k.any_refl = false;
     const int c = tid & (WS_COLS - 1);                             // column of the strip
     const int i = (int)blockIdx.x * (WS_COLS - 6) - 3 + c;         // column on the ghost-extended mesh
-    const int r0 = k.j0 - 3, rend = k.j1 + 4;                      // the Y group runs one row behind, output row = r - 4
+    const int r0 = k.j0 - 3, rend = k.j1 + 5;                      // the Y group runs behind, output row = r - 5
     double smx = 0.0, smy = 0.0;
     int flags = 0;
     __syncthreads();                                               // (the fill above is complete)
@@ -277,10 +286,11 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
         Y1 = Y0;
         YCarry cy;
         cy.gp1 = cy.gp2 = cy.gp3 = 0.0;
+        cy.q1 = 1.0; cy.q2 = cy.q3 = 0.0;
         cy.c1 = 1.0; cy.c2 = cy.c3 = cy.zC2 = cy.zC3 = cy.zS2 = cy.zS3 = 0.0;
         int r = r0;
-        // steady: interface ry-1/2 (ry = r-1) is a real one, output row r-4 >= j0 and away from the y edges
-        const int slo = max(k.j0 + 4, k.py ? 0 : 5), shi = min(rend - 1, g.ny);
+        // steady: interface ry-1/2 (ry = r-1) is a real one, output row r-5 >= j0 and away from the y edges
+        const int slo = max(k.j0 + 5, k.py ? 0 : 6), shi = min(rend - 1, g.ny);
         while (r < rend && (r < slo || (r & 1))) {
             if (r & 1) ws_ytick<1, false>(g, k, th, cy, Y0, Y1, r, o1, o2, o3); else ws_ytick<0, false>(g, k, th, cy, Y0, Y1, r, o1, o2, o3);
             ++r;
