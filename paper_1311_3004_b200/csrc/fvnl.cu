@@ -9,7 +9,6 @@
 #include <vector>
 
 #include "../../include/fvnl.h"
-#include "fvnl_pipe.cuh"
 #include "fvnl_ws.cuh"
 
 using namespace fvnl;
@@ -130,8 +129,8 @@ struct fvnl_ctx {
 };
 
 static const size_t MAX_SPANS = 1 << 16;
-static const int N_FUSED_VARIANTS = 12;
-static const int DEFAULT_VARIANT = 0;       // k_step_fused<128, 3>     // launch variants of the fused kernel (launch_fused)
+static const int N_FUSED_VARIANTS = 4;
+static const int DEFAULT_VARIANT = 0;       // k_step_ws<96, 160>     // launch variants of the fused kernel (launch_fused)
 
 // Event pair around one kernel launch (timing on only).
 struct SpanGuard {
@@ -363,21 +362,6 @@ static void launch_fused_t(fvnl_ctx* c, double** a, double** b) {
     k_step_fused<BX, MINB><<<grd, BX, fused_smem_bytes<BX>(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
 }
 
-template <int BX, int MINB>
-static void launch_pipe_t(fvnl_ctx* c, double** a, double** b) {
-    const Grid& g = c->g;
-    const int strips = (g.nx + (BX - 6) - 1) / (BX - 6);
-    const int rows = fused_rows(c, strips, 148 * MINB, 10);
-    const dim3 grd(strips, (g.ny + rows - 1) / rows);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_step_pipe<BX, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, pipe_smem_bytes<BX>());
-        attr_set = true;
-    }
-    SpanGuard sp(c, FVNL_TIMED_STEP);
-    k_step_pipe<BX, MINB><<<grd, BX, pipe_smem_bytes<BX>(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
-}
-
 template <int XREGS, int YREGS>
 static void launch_ws_t(fvnl_ctx* c, double** a, double** b) {
     const Grid& g = c->g;
@@ -395,22 +379,16 @@ static void launch_ws_t(fvnl_ctx* c, double** a, double** b) {
 }
 
 static void launch_fused(fvnl_ctx* c, double** a, double** b) {
+    // variants: 0 = warp-specialised kernel (default), 1 = the same without register re-balancing, 2.. = k_step_fused
     int variant = c->variant;
-    if (variant >= 8) {                     // the warp-specialised kernel has no analytic-source code (fvnl_ws.cuh)
+    if (variant <= 1) {                     // the warp-specialised kernel has no analytic-source code (fvnl_ws.cuh)
         for (int s = 0; s < 4; ++s)
-            if (c->g.side[s].kind == BC_SOURCE) variant = 0;
+            if (c->g.side[s].kind == BC_SOURCE) variant = 2;
     }
     switch (variant) {
-        case 8: launch_ws_t<128, 128>(c, a, b); break;
-        case 9: launch_ws_t<96, 160>(c, a, b); break;
-        case 11: launch_ws_t<168, 168>(c, a, b); break;
-        case 4: launch_pipe_t<128, 2>(c, a, b); break;
-        case 5: launch_pipe_t<128, 3>(c, a, b); break;
-        case 6: launch_pipe_t<256, 1>(c, a, b); break;
-        case 7: launch_pipe_t<160, 2>(c, a, b); break;
-        case 1: launch_fused_t<160, 3>(c, a, b); break;
-        case 2: launch_fused_t<96, 5>(c, a, b); break;
-        case 3: launch_fused_t<64, 7>(c, a, b); break;
+        case 0: launch_ws_t<96, 160>(c, a, b); break;
+        case 1: launch_ws_t<128, 128>(c, a, b); break;
+        case 3: launch_fused_t<256, 1>(c, a, b); break;
         default: launch_fused_t<128, 3>(c, a, b); break;
     }
 }

@@ -25,7 +25,7 @@ def run_both(w, steps=None, kernel=None, rows_per_block=None, chunks=None):
     fo = o.step(steps, w.value, w.mode)
     s = solver_from_workload(w, state=[torch.from_numpy(a) for a in state])
     if kernel is not None:
-        s.set_option(P.OPT_KERNEL, kernel)
+        select(s, kernel)
     if rows_per_block is not None:
         s.set_option(P.OPT_ROWS_PER_BLOCK, rows_per_block)
     fg = 0
@@ -33,6 +33,13 @@ def run_both(w, steps=None, kernel=None, rows_per_block=None, chunks=None):
         fg |= s.step(part, w.value, w.mode)
     gq = [a.cpu().numpy() for a in s.get_state()]
     return gq, o.get_state(), s.info(), o.info(), fg, fo
+
+
+def select(s, kernel):
+    """kernel = (FVNL_OPT_KERNEL value, FVNL_OPT_VARIANT value)."""
+    import paper_1311_3004_b200 as P
+    s.set_option(P.OPT_KERNEL, kernel[0])
+    s.set_option(P.OPT_VARIANT, kernel[1])
 
 
 def check(w, steps=None, tol=TOL, metric=parity_error, **kw):
@@ -48,10 +55,14 @@ def check(w, steps=None, tol=TOL, metric=parity_error, **kw):
     return err
 
 
-KERNELS = [0, 1]            # FVNL_KERNEL_DEFAULT (fused), FVNL_KERNEL_UNFUSED
+# (FVNL_OPT_KERNEL, FVNL_OPT_VARIANT): the warp-specialised one-pass kernel k_step_ws (the default; grids with an analytic
+# SOURCE edge are routed to k_step_fused by the library), the single-role one-pass kernel k_step_fused, and the
+# three-pass comparison kernels
+KERNELS = [(0, 0), (0, 2), (1, 0)]
+KIDS = ["ws", "fused", "unfused"]
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_p9_4x4_worked_step(kernel):
     """The 4x4 worked step of SURVEY.md 8(c) (tests/golden/p9_4x4.txt, written from an independent prototype of the
     same reading and reproduced by the oracle): periodic and extrapolation edges, fixed dt, source step on."""
@@ -63,7 +74,7 @@ def test_p9_4x4_worked_step(kernel):
     q3 = 0.003 * (((i * i + j) % 4) - 1.5)
     for bc, keys in ((P.PERIODIC, True), (P.EXTRAP, False)):
         s = P.Solver(4, 4, 1.0, 1.0, c0=1.0, rho0=1.0, beta=3.5, delta=0.05)
-        s.set_option(P.OPT_KERNEL, kernel)
+        select(s, kernel)
         for side in range(4):
             s.set_bc(side, bc)
         s.set_state(torch.from_numpy(q1), torch.from_numpy(q2.astype(float)), torch.from_numpy(q3))
@@ -80,47 +91,47 @@ def test_p9_4x4_worked_step(kernel):
             assert np.abs(c33 - np.array(g["extrap_cell_3_3"][0])).max() <= 1e-13
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_c1_piston_full(kernel):
     """C1 at full size: 512x4, 2000 steps, plane piston on x-lo, extrapolation x-hi, periodic y; q3 == 0 exactly."""
     check(W.c1_piston(), kernel=kernel)
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_c2_pulse_small(kernel):
     """C2 scaled to 300 x 200 (ragged against every tile size), sigma 8 cells, extrapolation edges, 150 steps:
     the pulse reaches and leaves through the edges."""
     check(W.c2_pulse(n=300, ny=200, sigma_cells=8.0, steps=150), kernel=kernel)
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_c3_random_small(kernel):
     """C3 scaled to 517 x 263 (prime-ish, several strips with a ragged tail), periodic, 200 steps as the full config."""
     check(W.c3_random(n=517, ny=263, steps=200, sig_lo=3.0, sig_hi=20.0), kernel=kernel)
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_c4_hifu_small(kernel):
     """C4 scaled: 640 x 256, focus at 160 cells, aperture 80 cells, 400 steps (packet enters, focuses, nonlinear)."""
     w = W.c4_hifu(nx=640, ny=256, steps=400, focus_cells=160.0, aperture_cells=80.0, tau0=-4.5)
     check(w, kernel=kernel)
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_c4_cw_source_small(kernel):
     """The continuous-wave reading of "time-harmonic" (SINE with an aperture and a focus)."""
     w = W.c4_hifu(nx=320, ny=192, steps=300, focus_cells=120.0, aperture_cells=60.0, tau0=0.0, shape=W.SINE)
     check(w, kernel=kernel)
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_c5_small_sizes(kernel):
     """C5 generator at 256^2 and 1000 x 96, nu_W = 0.9, 100 steps."""
     check(W.c5_sweep(n=256, steps=100), kernel=kernel)
     check(W.c5_sweep(n=1000, ny=96, steps=100), kernel=kernel)
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_taylor_dirichlet_edges(kernel):
     """C1-T (eta = 10): analytic (41) cells on all four sides, and with periodic y-edges.  The perturbation is 1e-7
     of the unit background, so one ulp of the state is already 2e-9 of it: the bar is 1e-7 (SURVEY.md 8(d) C1-T
@@ -130,7 +141,7 @@ def test_taylor_dirichlet_edges(kernel):
         check(w, steps=400, tol=1e-7, metric=parity_error_global, kernel=kernel)
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_reflecting_and_mixed_edges(kernel):
     """REFLECT on x-lo and y-hi, EXTRAP elsewhere, off-centre pulse, non-square cells (dx != dy)."""
     import paper_1311_3004_b200 as P
@@ -146,7 +157,7 @@ def test_reflecting_and_mixed_edges(kernel):
     check(w, kernel=kernel)
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_fixed_dt_mode_and_tiny_grids(kernel):
     """mode 0 (fixed dt) on the minimum grid 4x4 and on 5 x 4 / 4 x 7, periodic and extrapolation."""
     import paper_1311_3004_b200 as P
@@ -158,24 +169,24 @@ def test_fixed_dt_mode_and_tiny_grids(kernel):
             check(w, kernel=kernel)
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_restart_is_bitwise(kernel):
     """P10: N steps == k steps + get_state/get_info + set_state/set_clock + (N-k) steps, bit for bit; and splitting
     one fvnl_step call into several changes nothing."""
     import paper_1311_3004_b200 as P
     w = W.c3_random(n=200, ny=120, steps=40, sig_lo=3.0, sig_hi=10.0)
     a = solver_from_workload(w)
-    a.set_option(P.OPT_KERNEL, kernel)
+    select(a, kernel)
     a.step(40, w.value, 1)
     ref = [x.clone() for x in a.get_state()]
     b = solver_from_workload(w)
-    b.set_option(P.OPT_KERNEL, kernel)
+    select(b, kernel)
     b.step(10, w.value, 1)
     b.step(5, w.value, 1)
     mid = [x.clone() for x in b.get_state(host=True)]
     info = b.info()
     c = solver_from_workload(w)
-    c.set_option(P.OPT_KERNEL, kernel)
+    select(c, kernel)
     c.set_state(*mid)
     c.set_clock(info["t"], info["M"])
     c.step(25, w.value, 1)
@@ -184,14 +195,14 @@ def test_restart_is_bitwise(kernel):
     assert c.info()["t"] == a.info()["t"]
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_run_to_run_determinism(kernel):
     import paper_1311_3004_b200 as P
     w = W.c3_random(n=300, ny=300, steps=30, sig_lo=3.0, sig_hi=10.0)
     outs = []
     for _ in range(2):
         s = solver_from_workload(w)
-        s.set_option(P.OPT_KERNEL, kernel)
+        select(s, kernel)
         s.step(30, w.value, 1)
         outs.append([x.clone() for x in s.get_state()])
     for x, y in zip(*outs):
@@ -205,13 +216,14 @@ def test_fused_equals_unfused_to_rounding():
     outs = []
     for kernel in KERNELS:
         s = solver_from_workload(w)
-        s.set_option(P.OPT_KERNEL, kernel)
+        select(s, kernel)
         assert s.step(50, w.value, 1) == 0
         outs.append([x.cpu().numpy() for x in s.get_state()])
-    assert parity_error(outs[0], outs[1]) <= 1e-11
+    assert parity_error(outs[0], outs[2]) <= 1e-11
+    assert parity_error(outs[1], outs[2]) <= 1e-11
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
 def test_flags(kernel):
     """nu_W > 1 sets FVNL_ECFL; a state outside the real-eigenvalue region S sets FVNL_ENONREAL
     (PAPER.md:263-267); q1 <= 0 sets FVNL_ENONPOS -- same words as the oracle."""
@@ -259,3 +271,48 @@ def test_api_errors():
     rc, h = P.fvnl_create(64, 64, 1e-4, 1e-4, med, workspace_ptr=(ws.data_ptr() + 255) // 256 * 256, workspace_bytes=512)
     assert rc == P.EALLOC
     assert "CFL" in P.fvnl_strerror(P.ECFL)
+
+
+def _window_oracle(w, q0, i0, j0, size, margin, steps, dt):
+    """The oracle on a (size + 2 margin)^2 patch cut out of the full periodic grid (modular gather); after `steps` steps
+    with margin >= 3 steps + 3 the inner size^2 cells cannot have seen the patch edge (dependency cone: 3 cells / step)."""
+    from oracle.oracle import Oracle
+    n = size + 2 * margin
+    ii = (np.arange(i0 - margin, i0 - margin + n) % w.nx)
+    jj = (np.arange(j0 - margin, j0 - margin + n) % w.ny)
+    patch = [np.ascontiguousarray(q[jj][:, ii].cpu().numpy()) for q in q0]
+    o = Oracle(n, n, w.dx, w.dy, **w.medium, threads=0)
+    for side in range(4):
+        o.set_bc(side, 0)
+    o.set_state(*patch)
+    assert o.step(steps, dt, 0) == 0
+    return [a[margin:margin + size, margin:margin + size] for a in o.get_state()], (ii[margin:margin + size], jj[margin:margin + size])
+
+
+@pytest.mark.parametrize("n", [2048, 16384])
+def test_c5_full_size_sampled_windows(n):
+    """C5 at BASELINE.json's sizes (2048^2 and 16384^2), default kernel and launch configuration (what bench.py times):
+    the oracle cannot run the whole grid, so it recomputes WINDOWS of it -- 48^2 output cells each, cut out with a
+    margin wider than the dependency cone of the steps taken -- cell by cell; one window straddles the periodic corner.
+    Fixed dt (the CFL-mode dt depends on the whole grid), 5 steps.  Plus the property that holds at any size:
+    sum of q conserved under periodic edges."""
+    import paper_1311_3004_b200 as P
+    w = W.c5_sweep(n=n, steps=5)
+    q0 = w.init(device="cuda")
+    s = P.Solver(w.nx, w.ny, w.dx, w.dy, **w.medium)
+    for side, (kind, src) in enumerate(w.bc):
+        s.set_bc(side, kind, src)
+    s.set_state(*q0)
+    dt = 0.85 * w.dx / (w.medium["c0"] * 1.0011)
+    sums0 = [float(q.sum(dtype=torch.float64)) for q in q0]
+    assert s.step(5, dt, 0) == 0
+    out = s.get_state()
+    for m in range(3):
+        assert abs(float(out[m].sum(dtype=torch.float64)) - sums0[m]) <= 1e-12 * w.cells ** 0.5 * max(1.0, abs(sums0[m]) / w.cells) * 50
+    size, margin = 48, 20
+    worst = 0.0
+    for (i0, j0) in ((n - 24, n - 24), (n // 2 - 7, 3 * n // 4 + 11), (121, 377 % n)):
+        ref, (ii, jj) = _window_oracle(w, q0, i0, j0, size, margin, 5, dt)
+        got = [o_[torch.as_tensor(jj, device="cuda")][:, torch.as_tensor(ii, device="cuda")].cpu().numpy() for o_ in out]
+        worst = max(worst, parity_error(got, ref))
+    assert worst <= TOL, f"C5-{n}: windowed parity error {worst:.3e}"
