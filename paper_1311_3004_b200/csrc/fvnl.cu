@@ -89,6 +89,34 @@ __global__ void __launch_bounds__(256) k_prepass(Grid g, Clock* clk, const doubl
     block_flags_to(&clk->flags, flags);
 }
 
+// Boundary / source-injection kernel: the analytic ghost cells (41), (43a-d), piston of every SOURCE side at t_n
+// (readings A11, A13, A14, A16), three layers deep, into Grid::src.  One thread per record.
+__global__ void __launch_bounds__(128) k_sources(Grid g, const Clock* clk, double* __restrict__ out) {
+    const double t = clk->t;
+    size_t n = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    for (int sd = 0; sd < 4; ++sd) {
+        const size_t recs = src_side_doubles(g.nx, g.ny, sd) / 3;
+        if (n < recs) {
+            if (g.side[sd].kind != BC_SOURCE) return;
+            const int per = sd < 2 ? g.ny + 6 : g.nx;
+            const int l = (int)(n / per), m = (int)(n % per);
+            Q3 c;
+            bool in;
+            if (sd < 2) {
+                const int r = m - 3, i = sd == SIDE_XLO ? -1 - l : g.nx + l;
+                in = source_cell(g.side[sd], sd, g.c0, (r + 0.5) * g.dy, (i + 0.5) * g.dx, t, c);
+            } else {
+                const double x = (m + 0.5) * g.dx;
+                in = source_cell(g.side[sd], sd, g.c0, x, x, t, c);
+            }
+            double* o = out + src_off(g.nx, g.ny, sd) + 3 * n;
+            o[0] = in ? c.q1 : -1.0; o[1] = in ? c.q2 : 0.0; o[2] = in ? c.q3 : 0.0;
+            return;
+        }
+        n -= recs;
+    }
+}
+
 __global__ void k_fill(double* p, size_t n, double v) {
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = v;
 }
@@ -109,6 +137,7 @@ struct fvnl_ctx {
     void* ws;                   // workspace base
     bool own_ws;
     Clock* clk;                 // device clock
+    double* src;                // analytic ghost cells of the current step (k_sources)
     double* buf[2][3];          // two state buffers (ping-pong); cur = index of the current state
     int cur;
     double* star[3];            // unfused path only: Q* on the y-extended mesh, allocated on first use
@@ -167,7 +196,7 @@ static const size_t CLOCK_BYTES = 256;
 extern "C" size_t fvnl_workspace_bytes(int nx, int ny, int precision) {
     if (nx < 4 || ny < 4 || precision != 64) return 0;
     const size_t plane = align_up((size_t)nx * ny * sizeof(double), 256);
-    return CLOCK_BYTES + 6 * plane;
+    return CLOCK_BYTES + 6 * plane + align_up(src_off(nx, ny, 4) * sizeof(double), 256);
 }
 
 #define CK(call)                                         \
@@ -210,6 +239,7 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
     p += CLOCK_BYTES;
     for (int b = 0; b < 2; ++b)
         for (int k = 0; k < 3; ++k) { c->buf[b][k] = (double*)p; p += plane; }
+    c->src = (double*)p;
     if (cudaMallocHost((void**)&c->host_clk, sizeof(Clock)) != cudaSuccess) {
         (void)cudaGetLastError();
         if (c->own_ws) cudaFree(c->ws);
@@ -380,11 +410,7 @@ static void launch_ws_t(fvnl_ctx* c, double** a, double** b) {
 
 static void launch_fused(fvnl_ctx* c, double** a, double** b) {
     // variants: 0 = warp-specialised kernel (default), 1 = the same without register re-balancing, 2.. = k_step_fused
-    int variant = c->variant;
-    if (variant <= 1) {                     // the warp-specialised kernel has no analytic-source code (fvnl_ws.cuh)
-        for (int s = 0; s < 4; ++s)
-            if (c->g.side[s].kind == BC_SOURCE) variant = 2;
-    }
+    const int variant = c->variant;
     switch (variant) {
         case 0: launch_ws_t<96, 160>(c, a, b); break;
         case 1: launch_ws_t<128, 128>(c, a, b); break;
@@ -403,6 +429,9 @@ static int read_clock(fvnl_ctx* c) {
 extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
     if (!c || nsteps < 0 || !(value > 0.0) || (mode != 0 && mode != 1)) return FVNL_EARG;
     if (!c->have_state) return FVNL_ESTATE;
+    bool has_src = false;
+    for (int s = 0; s < 4; ++s) has_src = has_src || c->g.side[s].kind == BC_SOURCE;
+    c->g.src = has_src ? c->src : nullptr;
     const Grid& g = c->g;
     for (int ax = 0; ax < 2; ++ax)
         if ((g.side[2 * ax].kind == BC_PERIODIC) != (g.side[2 * ax + 1].kind == BC_PERIODIC)) return FVNL_EARG;
@@ -426,6 +455,11 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
         double** a = c->buf[c->cur];
         double** b = c->buf[c->cur ^ 1];
         if (c->kernel == FVNL_KERNEL_DEFAULT) {
+            if (has_src && c->variant <= 1) {                  // boundary / source-injection kernel for this step's t_n
+                const size_t recs = src_off(g.nx, g.ny, 4) / 3;
+                k_sources<<<(unsigned)((recs + 127) / 128), 128, 0, st>>>(g, c->clk, c->src);
+                c->launches += 1;
+            }
             launch_fused(c, a, b);
             c->launches += 1;
             c->cur ^= 1;

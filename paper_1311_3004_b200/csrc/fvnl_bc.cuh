@@ -22,7 +22,19 @@ struct Grid {
     int nx, ny;
     double dx, dy, c0, beta, delta;
     Side side[4];
+    const double* src;          // analytic ghost cells of this step, written by k_sources (null: no SOURCE side)
 };
+
+// Layout of Grid::src (doubles): three ghost layers per SOURCE side, layer l = distance - 1 from the edge; a record is
+// (q1, q2, q3), q1 <= 0 marking "outside the aperture" (the cell then behaves as EXTRAP).
+//   x-lo, x-hi : record (l, r), rows r = -3 .. ny+2   at  src_off(side) + 3 ((ny + 6) l + r + 3)
+//   y-lo, y-hi : record (l, i), columns i = 0 .. nx-1 at  src_off(side) + 3 (nx l + i)
+__host__ __device__ inline size_t src_side_doubles(int nx, int ny, int side) { return 9 * (size_t)(side < 2 ? ny + 6 : nx); }
+__host__ __device__ inline size_t src_off(int nx, int ny, int side) {
+    size_t o = 0;
+    for (int s = 0; s < side; ++s) o += src_side_doubles(nx, ny, s);
+    return o;
+}
 
 // Device-resident clock: the time step lives here so that no host synchronisation is needed between steps
 // (dt_n from the CFL number of step n-1).

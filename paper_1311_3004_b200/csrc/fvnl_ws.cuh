@@ -14,9 +14,10 @@
 //                        -> publish z of Q** for the neighbours' source step (parity r&1)        -> [bar ALL]
 // Arithmetic, ghost rules and validity masks are those of fvnl_fused.cuh.
 //
-// This kernel serves grids WITHOUT an analytic SOURCE edge (periodic / extrapolation / reflecting): ptxas 12.9 crashes
-// on setmaxnreg in a kernel that also calls the out-of-line source functions (sin / exp / tanh slow paths), and the
-// source cells sit in one strip only anyway.  fvnl_step launches k_step_fused when any edge is a SOURCE.
+// Analytic SOURCE edges: the ghost cells of the step are computed beforehand by the boundary kernel k_sources
+// (fvnl.cu) into Grid::src and only LOADED here (ptxas 12.9 crashes on setmaxnreg in a kernel that also calls the
+// out-of-line sin / exp / tanh paths, and evaluating them inside the march made the strip that owns the edge twice as
+// slow as the others).
 #pragma once
 #include "fvnl_fused.cuh"
 
@@ -66,9 +67,24 @@ __device__ __forceinline__ void ws_xtick(const Grid& g, const StepK& k, XThread&
         cp_async8(pd, q1 + idx); cp_async8(pd + WS_COLS * 8, q2 + idx); cp_async8(pd + 2 * WS_COLS * 8, q3 + idx);
         cp_async_commit();
     }
-    if ((th.special & 4) || (!STEADY && rm.neg3)) {                           // ghost column / row of a REFLECT side: rare
+    if ((th.special & 12) || (!STEADY && (rm.neg3 || rm.ysrc >= 0))) {        // ghost column / row with a rule: rare
         if (!STEADY && rm.neg3) a3 = -a3;
         if (th.special & 4) a2 = -a2;
+        bool done = false;                                                    // x rule first, then y rule (as load_ext)
+        if ((th.special & 8) && r >= -3 && r <= g.ny + 2) {
+            const int sd = th.cm.xsrc, l = sd == SIDE_XLO ? -1 - th.i : th.i - g.nx;
+            if (l < 3) {
+                const double* sp = g.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)(g.ny + 6) * l + r + 3);
+                if (sp[0] > 0.0) { a1 = sp[0]; a2 = sp[1]; a3 = sp[2]; done = true; }
+            }
+        }
+        if (!STEADY && !done && rm.ysrc >= 0) {
+            const int sd = rm.ysrc, l = sd == SIDE_YLO ? -1 - r : r - g.ny;
+            if (l < 3) {
+                const double* sp = g.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)g.nx * l + th.cm.col);
+                if (sp[0] > 0.0) { a1 = sp[0]; a2 = th.cm.neg2 ? -sp[1] : sp[1]; a3 = sp[2]; }
+            }
+        }
     }
     int tq = 0x7fffffff, td = 0x7fffffff;
     const Cx cx = cell_of(a1, a2, a3, tq);
@@ -105,9 +121,19 @@ __device__ __forceinline__ void ws_xtick(const Grid& g, const StepK& k, XThread&
     bar_all();                                                                // row r handed to the Y warps
 }
 
-// z of the one-deep ghost of Q** at a non-periodic, non-source edge: EXTRAP copies, REFLECT negates the normal velocity.
-__device__ __forceinline__ double2 ghost_z_plain(const Grid& g, int sd, double z2, double z3) {
-    if (g.side[sd].kind == BC_REFLECT) return sd < 2 ? make_double2(-z2, z3) : make_double2(z2, -z3);
+// z of the one-deep ghost of Q** at a non-periodic edge, from the z of the interior cell next to it (reading A9): EXTRAP
+// copies, REFLECT negates the normal velocity, SOURCE takes the analytic cell of layer 0 (record `m`: the row for an x
+// side, the column for a y side) if it lies inside the aperture.
+__device__ __forceinline__ double2 ghost_z_plain(const Grid& g, int sd, int m, double z2, double z3) {
+    const int kind = g.side[sd].kind;
+    if (kind == BC_REFLECT) return sd < 2 ? make_double2(-z2, z3) : make_double2(z2, -z3);
+    if (kind == BC_SOURCE) {
+        const double* sp = g.src + src_off(g.nx, g.ny, sd) + 3 * (size_t)(sd < 2 ? m + 3 : m);
+        if (sp[0] > 0.0) {
+            const double rc = rcp_o1(sp[0]);
+            return make_double2(sp[1] * rc, sp[2] * rc);
+        }
+    }
     return make_double2(z2, z3);
 }
 
@@ -150,8 +176,8 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
     cy.q1 = N.c.q1; cy.q2 = N.c.q2; cy.q3 = N.c.q3;                           // Q*(ry-2), y-form: next tick's lower row
     double2 zW = lds2(p + ws_arr2(11, R) - 16), zE = lds2(p + ws_arr2(11, R) + 16);   // z of row ry-4, published last tick
     if (th.special & 3) {
-        if (th.special & 1) zW = ghost_z_plain(g, SIDE_XLO, cy.zC2, cy.zC3);
-        if (th.special & 2) zE = ghost_z_plain(g, SIDE_XHI, cy.zC2, cy.zC3);
+        if (th.special & 1) zW = ghost_z_plain(g, SIDE_XLO, ry - 4, cy.zC2, cy.zC3);
+        if (th.special & 2) zE = ghost_z_plain(g, SIDE_XHI, ry - 4, cy.zC2, cy.zC3);
     }
     const double H2 = fma(k.k2, cy.zC2, fma(k.kapx, zE.x + zW.x, cy.c2));
     const double H3 = fma(k.k2, cy.zC3, fma(k.kapx, zE.y + zW.y, cy.c3));
@@ -163,8 +189,8 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
         double y2 = zN2 + cy.zS2, y3 = zN3 + cy.zS3;
         if (!STEADY && !k.py && (Ro == 0 || Ro == g.ny - 1)) {
             double2 lo = make_double2(cy.zS2, cy.zS3), hi = make_double2(zN2, zN3);
-            if (Ro == 0) lo = ghost_z_plain(g, SIDE_YLO, cy.zC2, cy.zC3);
-            if (Ro == g.ny - 1) hi = ghost_z_plain(g, SIDE_YHI, cy.zC2, cy.zC3);
+            if (Ro == 0) lo = ghost_z_plain(g, SIDE_YLO, th.i, cy.zC2, cy.zC3);
+            if (Ro == g.ny - 1) hi = ghost_z_plain(g, SIDE_YHI, th.i, cy.zC2, cy.zC3);
             y2 = hi.x + lo.x; y3 = hi.y + lo.y;
         }
         const double w2 = fma(k.kapy, y2, H2), w3 = fma(k.kapy, y3, H3);
