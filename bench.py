@@ -31,6 +31,9 @@ UNIT = "Gcell-updates/s"
 ALG_BYTES_PER_CELL = 48.0          # 3 fields x 8 B x (1 read + 1 write) per cell-update
 ALG_FLOP_PER_CELL = 404.0          # the oracle's formulas, division / sqrt = 1
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 lanes x FMA x 1965 MHz = 37.2
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel, from the committed `ncu --set full`
+# capture (profiles/r1_ws_ncu_summary.md): 6.590525 + 6.402814 GB at 16384^2, i.e. 48.4 B per cell-update
+NCU_TRAFFIC_BYTES = {"C5-16384": 12.993339e9}
 
 
 def reduce_max_ms(ms, dist, device):
@@ -276,6 +279,8 @@ def run_gpu(args):
     top = max(spans, key=lambda k: spans[k][0])
     top_ms = spans[top][0] / spans[top][1]
     share = spans[top][0] / ms
+    if args.traffic is None and args.kernel == "fused" and args.variant in (-1, 0):
+        args.traffic = NCU_TRAFFIC_BYTES.get(w.name)
     achieved = ALG_BYTES_PER_CELL * w.cells / (top_ms * 1e-3) / 1e9
     roofline_hbm = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
                     "frac": achieved / peak, "traffic": args.traffic, "peak_source": peak_src,

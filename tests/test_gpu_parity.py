@@ -51,6 +51,7 @@ def check(w, steps=None, tol=TOL, metric=parity_error, **kw):
     assert gi["M"] == pytest.approx(oi["M"], rel=1e-12)
     assert gi["cfl"] == pytest.approx(oi["cfl"], rel=1e-12)
     err = metric(gq, oq)
+    print(f"PARITY {w.name} {w.nx}x{w.ny} steps={gi['steps']} kernel={kw.get('kernel')} err={err:.3e} tol={tol:g}")
     assert err <= tol, f"{w.name}: parity error {err:.3e} > {tol}"
     return err
 
@@ -315,4 +316,5 @@ def test_c5_full_size_sampled_windows(n):
         ref, (ii, jj) = _window_oracle(w, q0, i0, j0, size, margin, 5, dt)
         got = [o_[torch.as_tensor(jj, device="cuda")][:, torch.as_tensor(ii, device="cuda")].cpu().numpy() for o_ in out]
         worst = max(worst, parity_error(got, ref))
+    print(f"PARITY C5-{n} windows {n}x{n} steps=5 kernel=default err={worst:.3e} tol={TOL:g}")
     assert worst <= TOL, f"C5-{n}: windowed parity error {worst:.3e}"
