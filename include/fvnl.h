@@ -133,13 +133,14 @@ int fvnl_get_state(fvnl_ctx* ctx, void* q1_dev_or_host, void* q2_dev_or_host, vo
 int fvnl_get_info(fvnl_ctx* ctx, double* t_s, double* last_dt_s, double* last_cfl, double* last_M,
                   long* steps_done);
 
-/* Kernel selection.  FVNL_KERNEL_DEFAULT: the fused one-pass step kernel (the product path).  FVNL_KERNEL_UNFUSED:
- * the three-pass form (x-sweep, y-sweep, source step as separate kernels through HBM; allocates one more
- * y-extended state with cudaMalloc on first use) -- a measured comparison point for "what fusion buys" and an
- * independently structured second implementation for cross-checks.  Same results up to rounding.
- * FVNL_OPT_ROWS_PER_BLOCK: rows one thread block of the fused kernel marches over (0 = automatic).
- * FVNL_OPT_VARIANT: launch variant of the fused kernel (block width / register budget; 0 = default; tuning aid,
- * results are identical for every variant). */
+/* Kernel selection (tuning and cross-check aid; results agree to rounding for every choice).
+ * FVNL_OPT_KERNEL:  FVNL_KERNEL_DEFAULT = the one-pass step kernel (each state array read once and written once per
+ *   step); FVNL_KERNEL_UNFUSED = the three-pass form (x-sweep, y-sweep, source step as separate kernels through HBM;
+ *   allocates one more y-extended state with cudaMalloc on first use) -- the measured "what fusion buys" point.
+ * FVNL_OPT_VARIANT (one-pass kernel): 0 = warp-specialised kernel k_step_ws with register re-balancing (default),
+ *   1 = the same without re-balancing, 2 = single-role kernel k_step_fused (128 threads), 3 = k_step_fused (256 threads).
+ * FVNL_OPT_ROWS_PER_BLOCK: rows one thread block of the one-pass kernel marches over (0 = automatic).
+ * FVNL_OPT_KERNEL_TIMING: see fvnl_get_kernel_time. */
 enum { FVNL_OPT_KERNEL = 0, FVNL_OPT_ROWS_PER_BLOCK = 1, FVNL_OPT_KERNEL_TIMING = 2, FVNL_OPT_VARIANT = 3 };
 enum { FVNL_KERNEL_DEFAULT = 0, FVNL_KERNEL_UNFUSED = 1 };
 int fvnl_set_option(fvnl_ctx* ctx, int option, int value);
