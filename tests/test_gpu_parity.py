@@ -318,3 +318,14 @@ def test_c5_full_size_sampled_windows(n):
         worst = max(worst, parity_error(got, ref))
     print(f"PARITY C5-{n} windows {n}x{n} steps=5 kernel=default err={worst:.3e} tol={TOL:g}")
     assert worst <= TOL, f"C5-{n}: windowed parity error {worst:.3e}"
+
+
+@pytest.mark.parametrize("rows", [4, 7, 64, 1000])
+@pytest.mark.parametrize("kernel", KERNELS[:2], ids=KIDS[:2])
+def test_rows_per_block_choices(kernel, rows):
+    """The one-pass kernels with forced chunk heights (down to chunks shorter than their own pipeline fill, and one
+    chunk for the whole grid): chunk seams, ragged last chunk, periodic wrap inside the halo of the first chunk."""
+    w = W.c3_random(n=300, ny=131, steps=25, sig_lo=3.0, sig_hi=12.0)
+    check(w, kernel=kernel, rows_per_block=rows)
+    w = W.c4_hifu(nx=260, ny=90, steps=40, focus_cells=60.0, aperture_cells=30.0, tau0=-1.0)
+    check(w, kernel=kernel, rows_per_block=rows)
