@@ -285,6 +285,7 @@ def run_gpu(args):
     roofline_hbm = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
                     "frac": achieved / peak, "traffic": args.traffic, "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": ALG_BYTES_PER_CELL * w.cells}
+    rc_probe, probe_tflops = P.fvnl_probe_fp64(torch.cuda.current_stream(dev).cuda_stream)
     tf = ALG_FLOP_PER_CELL * w.cells / (top_ms * 1e-3) / 1e12
     sm_mhz = clocks.get("sm_mhz") or 1965.0
     roofline = {"bound": "alu", "kernel": top, "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
@@ -292,6 +293,7 @@ def run_gpu(args):
                 "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x 1.965 GHz (DESIGN.md 7); fp64 vector pipe, "
                                "not in MEASURED_PEAKS.json",
                 "frac_at_observed_clock": tf / (FP64_PEAK_TFLOPS * sm_mhz / 1965.0),
+                "fp64_probe_tflops": probe_tflops if rc_probe == 0 else None,   # DFMA-only kernel, measured in this run
                 "algorithmic_flop_per_launch": ALG_FLOP_PER_CELL * w.cells, "ms_per_launch": top_ms,
                 "share_of_step": share,
                 "kernels": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1]} for k, v in spans.items()}}

@@ -155,6 +155,11 @@ int fvnl_set_option(fvnl_ctx* ctx, int option, int value);
 enum { FVNL_TIMED_STEP = 0, FVNL_TIMED_XSWEEP = 1, FVNL_TIMED_YSWEEP = 2, FVNL_TIMED_SOURCE = 3, FVNL_TIMED_KINDS = 4 };
 int fvnl_get_kernel_time(fvnl_ctx* ctx, int which, double* total_ms, long* launches);
 
+/* FP64-pipe probe for the roofline denominator: runs a register-only kernel of independent DFMA chains (16 warps per
+ * SM, 8 chains per thread) on the current device and stream and returns the achieved rate in TFLOP/s (FMA = 2 flop),
+ * best of three.  Needs no context.  Errors: FVNL_EARG, FVNL_ECUDA. */
+int fvnl_probe_fp64(void* cuda_stream, double* tflops);
+
 /* Number of kernels this context has launched so far (sweeps, pre-pass, packing); for bench accounting. */
 long fvnl_kernel_launches(const fvnl_ctx* ctx);
 

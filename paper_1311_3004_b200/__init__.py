@@ -72,6 +72,7 @@ def lib():
         L.fvnl_get_state.argtypes = [_vp, _vp, _vp, _vp, C.c_int]
         L.fvnl_get_info.argtypes = [_vp] + [C.POINTER(C.c_double)] * 4 + [C.POINTER(C.c_long)]
         L.fvnl_get_kernel_time.argtypes = [_vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_long)]
+        L.fvnl_probe_fp64.argtypes = [_vp, C.POINTER(C.c_double)]
         L.fvnl_kernel_launches.restype = C.c_long
         L.fvnl_kernel_launches.argtypes = [_vp]
         L.fvnl_strerror.restype = C.c_char_p
@@ -131,6 +132,12 @@ def fvnl_get_kernel_time(h, which):
     ms, n = C.c_double(), C.c_long()
     rc = lib().fvnl_get_kernel_time(h, int(which), C.byref(ms), C.byref(n))
     return rc, ms.value, n.value
+
+
+def fvnl_probe_fp64(cuda_stream=0):
+    v = C.c_double()
+    rc = lib().fvnl_probe_fp64(_vp(cuda_stream or None), C.byref(v))
+    return rc, v.value
 
 
 def fvnl_kernel_launches(h):

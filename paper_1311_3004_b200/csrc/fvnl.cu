@@ -517,6 +517,54 @@ extern "C" int fvnl_get_kernel_time(fvnl_ctx* c, int which, double* total_ms, lo
     return FVNL_OK;
 }
 
+// FP64-pipe probe: 8 independent DFMA chains per thread, 16 warps per SM, no memory traffic.
+__global__ void __launch_bounds__(128) k_probe_dfma(double* out, int iters, double a, double b) {
+    double x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = a + i + threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) x[i] = fma(x[i], b, a);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    if (s == 12345.678) out[0] = s;                       // never true: keeps the chains alive
+}
+
+extern "C" int fvnl_probe_fp64(void* cuda_stream, double* tflops) {
+    if (!tflops) return FVNL_EARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* d = nullptr;
+    CK(cudaMalloc((void**)&d, 8));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    const int iters = 8192, blocks = sms * 4, threads = 128;
+    k_probe_dfma<<<blocks, threads, 0, st>>>(d, 64, 1.0000001, 0.9999999);
+    float best = 1e30f;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(e0, st);
+        k_probe_dfma<<<blocks, threads, 0, st>>>(d, iters, 1.0000001, 0.9999999);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { (void)cudaGetLastError(); cudaFree(d); return FVNL_ECUDA; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    *tflops = 2.0 * (double)blocks * threads * iters * 64.0 / (best * 1e-3) / 1e12;
+    return FVNL_OK;
+}
+
 extern "C" long fvnl_kernel_launches(const fvnl_ctx* c) { return c ? c->launches : 0; }
 
 extern "C" const char* fvnl_strerror(int code) {
