@@ -154,7 +154,7 @@ struct ThreadK {
 // Carried between ticks besides the two YSets.
 struct Carry {
     double s1, s2, s3;                       // Q*(., r-1), left by the previous tick for the y-sweep
-    double gp1, gp2, gp3;                    // right-going part of the y-interface below the newest one, y-form
+    double gp1, gp2, gp3, gf1;               // right-going part (and F~, comp. 1) of the y-interface below the newest one
     double c1, c2, c3, zC2, zC3;             // Q**(r-3) and its z
     double zS2, zS3;                         // z of Q**(r-4)
 };
@@ -227,10 +227,10 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
     const double hb1 = N.w.al1 * d1 * A.rn1, hb2 = N.w.al2 * d2 * A.rn2;              // if N is A's upwind side
     const Fl G = flux2(A.w, hi_word(A.w.s1) < 0 ? hb1 : A.pb1, hi_word(A.w.s2) < 0 ? hb2 : A.pb2,
                        hi_word(A.w.v) < 0 ? N.w.al3 : A.pb3, k.lamy);
-    const double n1 = fma(-k.lamy, cy.gp1 + G.m1, b1o);                       // Q**(i, ry-2); physical order n1, n2, n3
+    const double n1 = update_q1(b1o, k.lamy, cy.gp1 + G.m1, cy.gf1, G.ft1);   // Q**(i, ry-2); physical order n1, n2, n3
     const double n3 = fma(-k.lamy, cy.gp2 + G.m2, b2o);
     const double n2 = fma(-k.lamy, cy.gp3 + G.m3, b3o);
-    cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3;
+    cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3; cy.gf1 = G.ft1;
     if (row_in) {
         th.mqx = min(th.mqx, tq); th.mdx = min(th.mdx, td);
         th.smx = dmax(th.smx, fabs(hi_word(w.v) < 0 ? w.s2 : w.s1));          // max(|s1|,|s2|) = |v| + a
@@ -253,7 +253,7 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
         const double b2 = k2.x * rdot(k2.y, k2r, w.s2, w.r32) * rn2;
         F = flux2(w, b1, b2, k3, k.lamx);
     }
-    sts2(p + sm_off<BX>(7), F.m1, F.m2); sts1(p + sm_off<BX>(8), F.m3);
+    sts2(p + sm_off<BX>(7), F.m1, F.m2); sts2(p + sm_off<BX>(8), F.m3, F.ft1);
     // source step, x part for row ry-3
     if (th.special & 3) {
         if (th.special & 1) zW = ghost_z(g, SIDE_XLO, (ry - 3 + 0.5) * g.dy, -0.5 * g.dx, k.t, cy.zC2, cy.zC3);
@@ -266,8 +266,9 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
     // ---- phase 3: Q*(i, r) for the next tick; source step (26): publish z of row ry-2, finish row R = ry-3 -------
     {
         const double2 gm = lds2(p + sm_off<BX>(7) + 16);
-        const double gm3 = lds1(p + sm_off<BX>(8) + 16);
-        cy.s1 = fma(-k.lamx, F.p1 + gm.x, a1);
+        const double2 gm3f = lds2(p + sm_off<BX>(8) + 16);
+        const double gm3 = gm3f.x;
+        cy.s1 = update_q1(a1, k.lamx, F.p1 + gm.x, F.ft1, gm3f.y);
         cy.s2 = fma(-k.lamx, F.p2 + gm.y, a2);
         cy.s3 = fma(-k.lamx, F.p3 + gm3, a3);
     }
@@ -340,7 +341,7 @@ k_step_fused(Grid g, Clock* clk, const double* __restrict__ q1,
     Y0.rn1 = Y0.rn2 = 0.5; Y0.pb1 = Y0.pb2 = Y0.pb3 = 0.0;
     Y1 = Y0;
     Carry cy;
-    cy.gp1 = cy.gp2 = cy.gp3 = 0.0;
+    cy.gp1 = cy.gp2 = cy.gp3 = cy.gf1 = 0.0;
     cy.s1 = 1.0; cy.s2 = cy.s3 = 0.0;
     cy.c1 = 1.0; cy.c2 = cy.c3 = cy.zC2 = cy.zC3 = cy.zS2 = cy.zS3 = 0.0;
 

@@ -115,6 +115,7 @@ __device__ __forceinline__ Waves riemann_x(const CellX& L, const CellX& R, doubl
 // with F~ of (30), limited by MC on the upwind neighbour's waves (readings A5, A6).
 struct Flux3 {
     double m1, m2, m3, p1, p2, p3;
+    double ft1;                         // first component of F~ alone (for the rounding order of the density update)
 };
 
 // `k`: this interface.  `u1`, `u2`, `u3`: (alpha, s, r3) of wave 1 / 2 and alpha of wave 3 at the interface that is
@@ -147,6 +148,7 @@ __device__ __forceinline__ Flux3 interface_flux(const Waves& k, double ual1, dou
     F.p1 = g1p + g2p;
     F.p2 = fma(g1p, k.s1, g2p * k.s2);
     F.p3 = fma(g1p, k.r31, fma(g2p, k.r32, g3p));
+    F.ft1 = f1 + f2;
     return F;
 }
 

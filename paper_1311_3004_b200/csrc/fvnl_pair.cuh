@@ -89,8 +89,9 @@ template <class T> struct CxT {       // a cell in sweep form: q2 normal, q3 tra
 template <class T> struct WvT {       // Riemann solution: W1 = al1 (1,s1,r31), W2 = al2 (1,s2,r32), W3 = (0,0,al3); v = s3
     T al1, s1, r31, al2, s2, r32, al3, v;
 };
-template <class T> struct FlT {       // left-going (m) and right-going (p) parts of an interface's contribution to (27)
-    T m1, m2, m3, p1, p2, p3;
+template <class T> struct FlT {       // left-going (m) and right-going (p) parts of an interface's contribution to (27),
+    T m1, m2, m3, p1, p2, p3;         // m = A^-DQ + F~, p = A^+DQ - F~; ft1 = first component of F~ alone
+    T ft1;
 };
 using Cx = CxT<double>;
 using Wv = WvT<double>;
@@ -170,7 +171,21 @@ __device__ __forceinline__ FlT<T> flux2(const WvT<T>& k, T b1, T b2, T b3, LAM l
     F.p1 = g1p + g2p;
     F.p2 = fma(g1p, k.s1, g2p * k.s2);
     F.p3 = fma(g1p, k.r31, fma(g2p, k.r32, g3p));
+    F.ft1 = f1 + f2;
     return F;
+}
+
+// The density component of the update (27).  q1 is of order one while its increment is of order of the perturbation, so
+// the two roundings of  (q - lam (A+DQ_l + A-DQ_r)) - lam (F~_r - F~_l)  (evaluated in this order) are the
+// largest round-off of a step by orders of magnitude, and a random walk of one-ulp differences over hundreds of steps
+// and 10^6..10^8 cells would by itself exceed the 1e-10 parity bar.  The CUDA path therefore rounds where the definition
+// rounds: two separate, uncontracted subtractions.  sum = p1_l + m1_r (both halves as produced by flux2), ft_l, ft_r =
+// first component of F~ at the two interfaces.
+__device__ __forceinline__ double update_q1(double q, double lam, double sum, double ft_l, double ft_r) {
+    const double s2 = __dsub_rn(ft_r, ft_l);                      // F~_r - F~_l
+    const double s1 = __dsub_rn(sum, s2);                         // A+DQ_l + A-DQ_r
+    const double u = __dsub_rn(q, __dmul_rn(lam, s1));
+    return __dsub_rn(u, __dmul_rn(lam, s2));
 }
 
 // ---- packing two scalar problems into the lanes of a pair and back ------------------------------------------------
@@ -186,7 +201,7 @@ __device__ __forceinline__ Cx lane_a(const CxT<V2>& c) { return Cx{c.q1.a, c.q2.
 __device__ __forceinline__ Cx lane_b(const CxT<V2>& c) { return Cx{c.q1.b, c.q2.b, c.q3.b, c.hz2.b, c.hz3.b}; }
 __device__ __forceinline__ Wv lane_a(const WvT<V2>& w) { return Wv{w.al1.a, w.s1.a, w.r31.a, w.al2.a, w.s2.a, w.r32.a, w.al3.a, w.v.a}; }
 __device__ __forceinline__ Wv lane_b(const WvT<V2>& w) { return Wv{w.al1.b, w.s1.b, w.r31.b, w.al2.b, w.s2.b, w.r32.b, w.al3.b, w.v.b}; }
-__device__ __forceinline__ Fl lane_a(const FlT<V2>& f) { return Fl{f.m1.a, f.m2.a, f.m3.a, f.p1.a, f.p2.a, f.p3.a}; }
-__device__ __forceinline__ Fl lane_b(const FlT<V2>& f) { return Fl{f.m1.b, f.m2.b, f.m3.b, f.p1.b, f.p2.b, f.p3.b}; }
+__device__ __forceinline__ Fl lane_a(const FlT<V2>& f) { return Fl{f.m1.a, f.m2.a, f.m3.a, f.p1.a, f.p2.a, f.p3.a, f.ft1.a}; }
+__device__ __forceinline__ Fl lane_b(const FlT<V2>& f) { return Fl{f.m1.b, f.m2.b, f.m3.b, f.p1.b, f.p2.b, f.p3.b, f.ft1.b}; }
 
 }  // namespace fvnl

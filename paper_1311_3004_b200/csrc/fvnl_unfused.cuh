@@ -55,7 +55,10 @@ __device__ __forceinline__ Q3 sweep_cell(const CellX c[5], double lam, double be
     sl = max_speed(w[1]);
     sr = max_speed(w[2]);
     Q3 o;
-    o.q1 = fma(-lam, F[0].p1 + F[1].m1, c[2].q1);
+    {   // density: rounded where (27) rounds, PAPER.md:161 (see update_q1 in fvnl_pair.cuh)
+        const double s2 = __dsub_rn(F[1].ft1, F[0].ft1), s1 = __dsub_rn(F[0].p1 + F[1].m1, s2);
+        o.q1 = __dsub_rn(__dsub_rn(c[2].q1, __dmul_rn(lam, s1)), __dmul_rn(lam, s2));
+    }
     o.q2 = fma(-lam, F[0].p2 + F[1].m2, c[2].q2);
     o.q3 = fma(-lam, F[0].p3 + F[1].m3, c[2].q3);
     if (not_finite(o.q1) || not_finite(o.q2) || not_finite(o.q3)) flags |= F_ENAN;

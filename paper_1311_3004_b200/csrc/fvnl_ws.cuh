@@ -114,9 +114,10 @@ __device__ __forceinline__ void ws_xtick(const Grid& g, const StepK& k, XThread&
         const double b2 = k2.x * rdot(k2.y, k2r, w.s2, w.r32) * rn2;
         const Fl F = flux2(w, b1, b2, k3, k.lamx);
         // the two halves of (27) for row r: what this interface sends left, and this column's own part
-        sts2(p + ws_arr2(7, P), F.m1, F.m2); sts1(p + ws_arr2(8, P), F.m3);
-        sts2(p + ws_arr2(9, P), fma(-k.lamx, F.p1, a1), fma(-k.lamx, F.p2, a2));
-        sts1(p + ws_arr2(10, P), fma(-k.lamx, F.p3, a3));
+        // (the density component goes over unrounded: q1, p1 and the first component of F~, see update_q1)
+        sts2(p + ws_arr2(7, P), F.m1, F.m2); sts2(p + ws_arr2(8, P), F.m3, F.ft1);
+        sts2(p + ws_arr2(9, P), a1, fma(-k.lamx, F.p2, a2));
+        sts2(p + ws_arr2(10, P), fma(-k.lamx, F.p3, a3), F.p1);
     }
     bar_all();                                                                // row r handed to the Y warps
 }
@@ -146,7 +147,7 @@ struct YThread {
 };
 
 struct YCarry {
-    double gp1, gp2, gp3;                    // right-going part of the y-interface below the newest one, y-form
+    double gp1, gp2, gp3, gf1;               // right-going part (and F~, comp. 1) of the y-interface below the newest one
     double q1, q2, q3;                       // Q*(., ry-3), y-form
     double c1, c2, c3, zC2, zC3;             // Q**(ry-4) and its z
     double zS2, zS3;                         // z of Q**(ry-5)
@@ -169,10 +170,10 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
     const int ry = r - 1;
     // ---- chain 2: flux of B, Q**(., ry-3), source step ----------------------------------------------------------------
     const Fl G = flux2(N.w, N.pb1, N.pb2, N.pb3, k.lamy);                     // N still holds B
-    const double n1 = fma(-k.lamy, cy.gp1 + G.m1, cy.q1);                     // Q**(i, ry-3); physical order n1, n2, n3
+    const double n1 = update_q1(cy.q1, k.lamy, cy.gp1 + G.m1, cy.gf1, G.ft1); // Q**(i, ry-3); physical order n1, n2, n3
     const double n3 = fma(-k.lamy, cy.gp2 + G.m2, cy.q2);
     const double n2 = fma(-k.lamy, cy.gp3 + G.m3, cy.q3);
-    cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3;
+    cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3; cy.gf1 = G.ft1;
     cy.q1 = N.c.q1; cy.q2 = N.c.q2; cy.q3 = N.c.q3;                           // Q*(ry-2), y-form: next tick's lower row
     double2 zW = lds2(p + ws_arr2(11, R) - 16), zE = lds2(p + ws_arr2(11, R) + 16);   // z of row ry-4, published last tick
     if (th.special & 3) {
@@ -207,8 +208,10 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
     double s1, s2, s3;                                                        // Q*(i, ry): the update (27) completed
     {
         const double2 u = lds2(p + ws_arr2(9, R)), gm = lds2(p + ws_arr2(7, R) + 16);
-        const double u3 = lds1(p + ws_arr2(10, R)), gm3 = lds1(p + ws_arr2(8, R) + 16);
-        s1 = fma(-k.lamx, gm.x, u.x); s2 = fma(-k.lamx, gm.y, u.y); s3 = fma(-k.lamx, gm3, u3);
+        const double2 u3 = lds2(p + ws_arr2(10, R)), gm3 = lds2(p + ws_arr2(8, R) + 16);
+        const double ft_own = lds1(p + ws_arr2(8, R) + 8);
+        s1 = update_q1(u.x, k.lamx, u3.y + gm.x, ft_own, gm3.y);
+        s2 = fma(-k.lamx, gm.y, u.y); s3 = fma(-k.lamx, gm3.x, u3.x);
     }
     int tqy = 0x7fffffff, tdy = 0x7fffffff;
     N.c = cell_of(s1, s3, s2, tqy);                                           // positions 2,3 switched
@@ -311,7 +314,7 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
         Y0.rn1 = Y0.rn2 = 0.5; Y0.pb1 = Y0.pb2 = Y0.pb3 = 0.0;
         Y1 = Y0;
         YCarry cy;
-        cy.gp1 = cy.gp2 = cy.gp3 = 0.0;
+        cy.gp1 = cy.gp2 = cy.gp3 = cy.gf1 = 0.0;
         cy.q1 = 1.0; cy.q2 = cy.q3 = 0.0;
         cy.c1 = 1.0; cy.c2 = cy.c3 = cy.zC2 = cy.zC3 = cy.zS2 = cy.zS3 = 0.0;
         int r = r0;

@@ -329,3 +329,83 @@ def test_rows_per_block_choices(kernel, rows):
     check(w, kernel=kernel, rows_per_block=rows)
     w = W.c4_hifu(nx=260, ny=90, steps=40, focus_cells=60.0, aperture_cells=30.0, tau0=-1.0)
     check(w, kernel=kernel, rows_per_block=rows)
+
+
+def test_c2_full_size():
+    """C2 at BASELINE.json's full size and step count (1024^2, 500 steps, extrapolation edges, nu_W = 0.9): the oracle
+    runs the whole problem (about half a minute on the box's cores); element-by-element parity plus the mirror symmetry
+    of the centred pulse (P4) on the GPU result."""
+    w = W.c2_pulse()
+    err = check(w)
+    assert err <= TOL
+    s = solver_from_workload(w)
+    assert s.step(w.steps, w.value, w.mode) == 0
+    q1, q2, q3 = [a.cpu().numpy() for a in s.get_state()]
+    # the oracle is mirror symmetric to round-off (pin P4); the CUDA path is within TOL of it, hence within 2 TOL of its
+    # own mirror image
+    amp = np.abs(q1 - 1.0).max()
+    assert np.abs(q1 - q1[:, ::-1]).max() <= 2 * TOL * amp and np.abs(q1 - q1[::-1, :]).max() <= 2 * TOL * amp
+    assert np.abs(q2 + q2[:, ::-1]).max() <= 2 * TOL * np.abs(q2).max()
+    assert np.abs(q3 + q3[::-1, :]).max() <= 2 * TOL * np.abs(q3).max()
+
+
+def test_c3_full_size_sampled_windows():
+    """C3 at full size (4096^2, periodic, nu_W = 0.8): 200 steps in CFL mode for the property that holds at any size
+    (sum of q conserved), and oracle-recomputed windows over 6 fixed-dt steps as for C5."""
+    import paper_1311_3004_b200 as P
+    w = W.c3_random()
+    q0 = w.init(device="cuda")
+    s = P.Solver(w.nx, w.ny, w.dx, w.dy, **w.medium)
+    for side, (kind, src) in enumerate(w.bc):
+        s.set_bc(side, kind, src)
+    s.set_state(*q0)
+    sums0 = [float(q.sum(dtype=torch.float64)) for q in q0]
+    assert s.step(w.steps, w.value, w.mode) == 0
+    assert abs(s.info()["cfl"] - w.value) < 1e-3
+    for m, q in enumerate(s.get_state()):
+        assert abs(float(q.sum(dtype=torch.float64)) - sums0[m]) <= 4e-8 * (1.0 if m else 1.0)
+    s.set_state(*q0)
+    dt = 0.75 * w.dx / (w.medium["c0"] * 1.0011)
+    assert s.step(6, dt, 0) == 0
+    out = s.get_state()
+    worst = 0.0
+    for (i0, j0) in ((w.nx - 20, 5), (1777, 3001)):
+        ref, (ii, jj) = _window_oracle(w, q0, i0, j0, 48, 24, 6, dt)
+        got = [o_[torch.as_tensor(jj, device="cuda")][:, torch.as_tensor(ii, device="cuda")].cpu().numpy() for o_ in out]
+        worst = max(worst, parity_error(got, ref))
+    print(f"PARITY C3 windows {w.nx}x{w.ny} steps=6 kernel=default err={worst:.3e} tol={TOL:g}")
+    assert worst <= TOL
+
+
+def test_c4_full_size_source_window():
+    """C4 at full size (8192 x 2048, focused packet source on x-lo, nu_W = 0.8): 240 steps, by which the packet has entered
+    (tau from -9.1 to -3.1 periods).  The oracle recomputes a patch that contains the source edge around the centre of
+    the aperture, wide enough that the compared 64 x 64 cells at the edge cannot have seen the patch's other edges
+    (3 cells per step); fixed dt so that both take the same steps."""
+    import paper_1311_3004_b200 as P
+    from oracle.oracle import Oracle
+    w = W.c4_hifu()
+    steps, size = 240, 64
+    margin = 3 * steps + 8
+    s = solver_from_workload(w, state=w.init(device="cuda"))
+    dt = 0.8 * w.dx / (w.medium["c0"] * 1.003)
+    assert s.step(steps, dt, 0) == 0
+    out = s.get_state()
+    jc = w.ny // 2
+    j_lo = max(0, jc - size // 2 - margin)
+    j_hi = min(w.ny, jc + size // 2 + margin)
+    nyp, nxp = j_hi - j_lo, size + margin
+    o = Oracle(nxp, nyp, w.dx, w.dy, **w.medium, threads=0)
+    src = dict(w.bc[0][1])
+    src["centre_m"] = src["centre_m"] - j_lo * w.dy                 # the aperture in the patch's own y coordinate
+    o.set_bc(0, P.SOURCE, src)
+    for side in (1, 2, 3):
+        o.set_bc(side, P.EXTRAP)
+    o.set_state(np.ones((nyp, nxp)), np.zeros((nyp, nxp)), np.zeros((nyp, nxp)))
+    assert o.step(steps, dt, 0) == 0
+    ref = [a[jc - size // 2 - j_lo: jc + size // 2 - j_lo, :size] for a in o.get_state()]
+    got = [a[jc - size // 2: jc + size // 2, :size].cpu().numpy() for a in out]
+    assert np.abs(ref[0] - 1.0).max() > 1e-5                           # the packet is there
+    err = parity_error(got, ref)
+    print(f"PARITY C4 source window {w.nx}x{w.ny} steps={steps} kernel=default err={err:.3e} tol={TOL:g}")
+    assert err <= TOL
