@@ -409,3 +409,33 @@ def test_c4_full_size_source_window():
     err = parity_error(got, ref)
     print(f"PARITY C4 source window {w.nx}x{w.ny} steps={steps} kernel=default err={err:.3e} tol={TOL:g}")
     assert err <= TOL
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
+def test_extreme_aspect_ratios(kernel):
+    """One very long row of strips (100 003 x 4) and one very tall strip (4 x 20 011): many strips with a ragged last one,
+    a grid narrower than a strip's halo, many chunks."""
+    import paper_1311_3004_b200 as P
+    for nx, ny in ((100003, 4), (4, 20011)):
+        for bc in (P.PERIODIC, P.EXTRAP):
+            w = W.c3_random(n=nx, ny=ny, steps=12, sig_lo=2.0, sig_hi=6.0, seed=99 + nx)
+            w.bc = [(bc, None)] * 4
+            check(w, kernel=kernel)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
+def test_equilibrium_is_a_fixed_point(kernel):
+    """The degenerate case: Q = Q_eq stays Q_eq bit for bit under every passive edge kind (all waves vanish identically),
+    M = 1/dx exactly (|s| = 1 at rest), and zero steps change nothing."""
+    import paper_1311_3004_b200 as P
+    for bc in (P.PERIODIC, P.EXTRAP, P.REFLECT):
+        s = P.Solver(150, 37, 1e-4, 1e-4, c0=1500.0, rho0=1000.0, beta=3.5, delta=4.3e-6)
+        select(s, kernel)
+        for side in range(4):
+            s.set_bc(side, bc)
+        assert s.step(0, 0.9, 1) == 0
+        assert s.step(25, 0.9, 1) == 0
+        q1, q2, q3 = s.get_state()
+        assert torch.equal(q1, torch.ones_like(q1)) and not q2.any() and not q3.any()
+        info = s.info()
+        assert info["steps"] == 25 and info["M"] == pytest.approx(1.0 / 1e-4, rel=1e-15) and info["cfl"] == pytest.approx(0.9, rel=1e-14)
