@@ -118,7 +118,8 @@ int fvnl_set_clock(fvnl_ctx* ctx, double t_s, double last_M);
  *   mode 1: value = nu_W; dt_n = nu_W/(c0*M_{n-1}), M = max over all x-interfaces of |s|/dx and y-interfaces of
  *           |s|/dy met during the previous step; first step: a pre-pass over the current state.
  *           No step is rejected; a step that ran with nu_n = c0*dt_n*M_n > 1 sets FVNL_ECFL.
- * The steps are queued on the stream without host synchronisation (dt lives on the device); the call then reads
+ * The steps are queued on the stream without host synchronisation (dt lives on the device; on grids of at most 2^18
+ * cells pairs of steps are replayed from a CUDA graph captured on first use); the call then reads
  * back 64 bytes {flags, t, dt, M, steps} and returns the OR of the sticky device flags (0 = clean).  With flags
  * set the state is undefined but readable.
  * Errors: FVNL_EARG (nsteps < 0, value <= 0, bad mode, lone PERIODIC, mode 0 with delta*dt*(1/dx^2+1/dy^2) > 1/2),

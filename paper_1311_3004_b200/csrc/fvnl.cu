@@ -149,6 +149,12 @@ struct fvnl_ctx {
     int rows_per_block;         // fused kernel: rows per chunk (0 = automatic)
     int variant;                // fused kernel: launch variant
     long launches;
+    // CUDA graph of two consecutive steps (state A -> B -> A), for grids so small that launches dominate
+    cudaStream_t gstream;       // capture stream (never executes anything)
+    cudaGraphExec_t gexec;
+    bool gvalid;
+    double gvalue;
+    int gmode, gcur, gvariant, grows;
     // opt-in per-kernel timing (FVNL_OPT_KERNEL_TIMING): event pairs around the sweep kernels, resolved on demand
     bool timing;
     struct Span { int id; cudaEvent_t a, b; };
@@ -270,6 +276,8 @@ extern "C" void fvnl_destroy(fvnl_ctx* c) {
     delete c->spans;
     for (int k = 0; k < 3; ++k)
         if (c->star[k]) cudaFree(c->star[k]);
+    if (c->gexec) cudaGraphExecDestroy(c->gexec);
+    if (c->gstream) cudaStreamDestroy(c->gstream);
     if (c->host_clk) cudaFreeHost(c->host_clk);
     if (c->own_ws && c->ws) cudaFree(c->ws);
     (void)cudaGetLastError();
@@ -288,11 +296,13 @@ extern "C" int fvnl_set_bc(fvnl_ctx* c, int side, int kind, const fvnl_source* s
         d.half_aperture_m = s->half_aperture_m; d.t0_s = s->t0_s; d.steep = s->steep;
     }
     c->g.side[side] = d;
+    c->gvalid = false;
     return FVNL_OK;
 }
 
 extern "C" int fvnl_set_option(fvnl_ctx* c, int option, int value) {
     if (!c) return FVNL_EARG;
+    c->gvalid = false;
     if (option == FVNL_OPT_KERNEL) {
         if (value != FVNL_KERNEL_DEFAULT && value != FVNL_KERNEL_UNFUSED) return FVNL_EARG;
         c->kernel = value;
@@ -426,6 +436,24 @@ static int read_clock(fvnl_ctx* c) {
     return FVNL_OK;
 }
 
+static const size_t GRAPH_MAX_CELLS = 1u << 18;      // below this a step is a few microseconds: launches dominate
+
+// One time step of the default path on c->stream: boundary kernel (if any edge is a SOURCE), step kernel, clock kernel.
+static void default_step(fvnl_ctx* c, bool has_src, double value, int mode, int more) {
+    const Grid& g = c->g;
+    double** a = c->buf[c->cur];
+    double** b = c->buf[c->cur ^ 1];
+    if (has_src && c->variant <= 1) {                           // this step's analytic ghost cells, at t_n
+        const size_t recs = src_off(g.nx, g.ny, 4) / 3;
+        k_sources<<<(unsigned)((recs + 127) / 128), 128, 0, c->stream>>>(g, c->clk, c->src);
+        c->launches += 1;
+    }
+    launch_fused(c, a, b);
+    c->cur ^= 1;
+    k_clock_end<<<1, 1, 0, c->stream>>>(g, c->clk, value, mode, more);
+    c->launches += 2;
+}
+
 extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
     if (!c || nsteps < 0 || !(value > 0.0) || (mode != 0 && mode != 1)) return FVNL_EARG;
     if (!c->have_state) return FVNL_ESTATE;
@@ -451,19 +479,48 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
         const int rc = ensure_star(c);
         if (rc) return rc;
     }
-    for (long n = 0; n < nsteps; ++n) {
+    long n = 0;
+    // Launch-bound grids: replay a captured graph of two steps (A -> B -> A) while at least three steps remain; the last
+    // steps (the final one computes no dt for a successor) go out as plain launches below.
+    if (c->kernel == FVNL_KERNEL_DEFAULT && !c->timing && c->n <= GRAPH_MAX_CELLS && nsteps >= 4) {
+        if (!c->gvalid || c->gvalue != value || c->gmode != mode || c->gcur != c->cur || c->gvariant != c->variant ||
+            c->grows != c->rows_per_block) {
+            if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+            c->gvalid = false;
+            if (!c->gstream && cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking) != cudaSuccess) c->gstream = nullptr;
+            cudaGraph_t graph = nullptr;
+            if (c->gstream && cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeRelaxed) == cudaSuccess) {
+                const cudaStream_t user = c->stream;
+                c->stream = c->gstream;
+                const long l0 = c->launches;
+                for (int half = 0; half < 2; ++half) default_step(c, has_src, value, mode, 1);
+                c->launches = l0;                               // nothing ran: the capture only records
+                c->stream = user;
+                if (cudaStreamEndCapture(c->gstream, &graph) == cudaSuccess && graph &&
+                    cudaGraphInstantiate(&c->gexec, graph, 0) == cudaSuccess) {
+                    c->gvalid = true; c->gvalue = value; c->gmode = mode; c->gcur = c->cur; c->gvariant = c->variant;
+                    c->grows = c->rows_per_block;
+                }
+                if (graph) cudaGraphDestroy(graph);
+            }
+            (void)cudaGetLastError();
+        }
+        if (c->gvalid) {
+            const int per_step = (has_src && c->variant <= 1 ? 1 : 0) + 2;
+            for (; n + 3 <= nsteps; n += 2) {
+                CK(cudaGraphLaunch(c->gexec, st));
+                c->launches += 2 * per_step;
+            }
+        }
+    }
+    for (; n < nsteps; ++n) {
+        if (c->kernel == FVNL_KERNEL_DEFAULT) {
+            default_step(c, has_src, value, mode, n + 1 < nsteps ? 1 : 0);
+            continue;
+        }
         double** a = c->buf[c->cur];
         double** b = c->buf[c->cur ^ 1];
-        if (c->kernel == FVNL_KERNEL_DEFAULT) {
-            if (has_src && c->variant <= 1) {                  // boundary / source-injection kernel for this step's t_n
-                const size_t recs = src_off(g.nx, g.ny, 4) / 3;
-                k_sources<<<(unsigned)((recs + 127) / 128), 128, 0, st>>>(g, c->clk, c->src);
-                c->launches += 1;
-            }
-            launch_fused(c, a, b);
-            c->launches += 1;
-            c->cur ^= 1;
-        } else {
+        {
             const dim3 grdx((g.nx + 255) / 256, g.ny + 4);
             { SpanGuard sp(c, FVNL_TIMED_XSWEEP);
               k_xsweep_unfused<<<grdx, blk, 0, st>>>(g, c->clk, a[0], a[1], a[2], c->star[0], c->star[1], c->star[2]); }
