@@ -332,7 +332,8 @@ def run_gpu(args):
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": w.name, "grid": [w.nx, w.ny], "cells": w.cells, "bc": [k for k, _ in w.bc],
-                   "nu_W": w.value, "kernel": args.kernel, "variant": args.variant, "rows_per_block": args.rows, "state_bytes": 24 * w.cells,
+                   "nu_W": w.value, "kernel": top if args.kernel == "fused" else "three-pass (" + top + " is the slowest of the three)",
+                   "variant": args.variant, "rows_per_block": args.rows, "state_bytes": 24 * w.cells,
                    "l2": "state larger than L2, no flush" if 24 * w.cells > 4 * 126e6 else "state near/below L2 size",
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "flags": int(flags),
                    "t_end_s": info["t"], "last_cfl": info["cfl"]},
