@@ -439,3 +439,24 @@ def test_equilibrium_is_a_fixed_point(kernel):
         assert torch.equal(q1, torch.ones_like(q1)) and not q2.any() and not q3.any()
         info = s.info()
         assert info["steps"] == 25 and info["M"] == pytest.approx(1.0 / 1e-4, rel=1e-15) and info["cfl"] == pytest.approx(0.9, rel=1e-14)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
+def test_sources_on_every_side(kernel):
+    """Focused packet on x-hi, plane piston on y-lo, continuous focused source on y-hi, Taylor profile on x-lo (each with
+    extrapolation or reflection elsewhere): the side-dependent signs of (43b,c) and all four blocks of the boundary
+    kernel's buffer."""
+    import paper_1311_3004_b200 as P
+    dx = W.LAMBDA_1MHZ / 32
+    base = dict(shape=P.PACKET, amp=4e-4, freq_hz=1e6, focus_m=50 * dx, centre_m=70 * dx, half_aperture_m=30 * dx,
+                t0_s=-1.5e-6, steep=0.0)
+    cases = []
+    w = W.c2_pulse(n=180, ny=140, sigma_cells=5.0, steps=120, amp=2e-4)
+    w.bc = [(P.EXTRAP, None), (P.SOURCE, dict(base)), (P.REFLECT, None), (P.EXTRAP, None)]
+    cases.append(w)
+    w = W.c2_pulse(n=150, ny=170, sigma_cells=5.0, steps=120, amp=2e-4)
+    w.bc = [(P.EXTRAP, None), (P.EXTRAP, None), (P.SOURCE, dict(base, shape=P.SINE, focus_m=0.0, half_aperture_m=0.0, t0_s=0.0)),
+            (P.SOURCE, dict(base, shape=P.SINE, t0_s=0.0, centre_m=80 * dx))]
+    cases.append(w)
+    for w in cases:
+        check(w, kernel=kernel)
