@@ -172,7 +172,8 @@ def c4_hifu(nx=8192, ny=2048, steps=4000, focus_cells=2048.0, aperture_cells=640
     src = _src(shape, amp=amp, freq_hz=1.0e6, focus_m=F, centre_m=ny * dx / 2.0, half_aperture_m=a,
                t0_s=tau0 / 1.0e6)
     return Workload("C4", nx, ny, dx, dx, med, [(SOURCE, src), (EXTRAP, None), (EXTRAP, None), (EXTRAP, None)],
-                    1, nu_w, steps, _equilibrium(nx, ny), "HIFU-like packet", extra=dict(tau0=tau0))
+                    1, nu_w, steps, _equilibrium(nx, ny), "HIFU-like packet",
+                    extra=dict(tau0=tau0, focus_cells=focus_cells, aperture_cells=aperture_cells))
 
 
 BY_NAME = {
