@@ -103,13 +103,15 @@ void fvnl_destroy(fvnl_ctx* ctx);
 int fvnl_set_bc(fvnl_ctx* ctx, int side, int kind, const fvnl_source* src_or_null);
 
 /* Copy a state in (three planes of nx*ny doubles).  Resets the sticky flags and the lagged maximum M (the next
- * CFL-mode step starts with the pre-pass), keeps t.  Asynchronous on the stream for device input; for host input
- * the buffers may be reused when the call returns. */
+ * CFL-mode step starts with the pre-pass), keeps t.  Device input: asynchronous, everything (copies and the clock reset)
+ * is queued on the stream and the call returns at once.  Host input: the call synchronises the stream, so the buffers may
+ * be reused when it returns. */
 int fvnl_set_state(fvnl_ctx* ctx, const void* q1_dev_or_host, const void* q2_dev_or_host,
                    const void* q3_dev_or_host, int on_device);
 
 /* Set the clock: simulation time t [s] and the lagged maximum M [1/m] of the previous step.
- * last_M <= 0: recompute M by the pre-pass on the current state at the next CFL-mode step.
+ * last_M <= 0: M unknown -- the next CFL-mode step recomputes it by the pre-pass on the state as it is then, unless a
+ * fixed-dt step has been taken in between (M is then that step's).  Asynchronous (queued on the stream).
  * (t, M) from fvnl_get_info + the state from fvnl_get_state restart a run bit-exactly. */
 int fvnl_set_clock(fvnl_ctx* ctx, double t_s, double last_M);
 
@@ -118,10 +120,11 @@ int fvnl_set_clock(fvnl_ctx* ctx, double t_s, double last_M);
  *   mode 1: value = nu_W; dt_n = nu_W/(c0*M_{n-1}), M = max over all x-interfaces of |s|/dx and y-interfaces of
  *           |s|/dy met during the previous step; first step: a pre-pass over the current state.
  *           No step is rejected; a step that ran with nu_n = c0*dt_n*M_n > 1 sets FVNL_ECFL.
- * The steps are queued on the stream without host synchronisation (dt lives on the device; on grids of at most 2^18
- * cells pairs of steps are replayed from a CUDA graph captured on first use); the call then reads
- * back 64 bytes {flags, t, dt, M, steps} and returns the OR of the sticky device flags (0 = clean).  With flags
- * set the state is undefined but readable.
+ * The steps are queued on the stream without host synchronisation, ONE kernel launch per time step: dt lives on the
+ * device, and the thread block of the step kernel that finishes last ends the step (M_n, nu_n, t, the next dt, the
+ * analytic ghost cells of the next step).  On grids of at most 2^18 cells pairs of steps are replayed from a CUDA graph
+ * captured on first use.  The call then reads back the clock {flags, t, dt, M, steps} and returns the OR of the sticky
+ * device flags (0 = clean).  With flags set the state is undefined but readable.
  * Errors: FVNL_EARG (nsteps < 0, value <= 0, bad mode, lone PERIODIC, mode 0 with delta*dt*(1/dx^2+1/dy^2) > 1/2),
  * FVNL_ECUDA. */
 int fvnl_step(fvnl_ctx* ctx, long nsteps, double value, int mode);
@@ -138,8 +141,8 @@ int fvnl_get_info(fvnl_ctx* ctx, double* t_s, double* last_dt_s, double* last_cf
  * FVNL_OPT_KERNEL:  FVNL_KERNEL_DEFAULT = the one-pass step kernel (each state array read once and written once per
  *   step); FVNL_KERNEL_UNFUSED = the three-pass form (x-sweep, y-sweep, source step as separate kernels through HBM;
  *   allocates one more y-extended state with cudaMalloc on first use) -- the measured "what fusion buys" point.
- * FVNL_OPT_VARIANT (one-pass kernel): 0 = warp-specialised kernel k_step_ws with register re-balancing (default),
- *   1 = the same without re-balancing, 2 = single-role kernel k_step_fused (128 threads), 3 = k_step_fused (256 threads).
+ * FVNL_OPT_VARIANT (one-pass kernel): 0 = warp-specialised kernel k_step_ws (default), 1 = single-role kernel
+ *   k_step_fused (one thread does both sweeps of its column; evaluates analytic edge cells in place).
  * FVNL_OPT_ROWS_PER_BLOCK: rows one thread block of the one-pass kernel marches over (0 = automatic).
  * FVNL_OPT_KERNEL_TIMING: see fvnl_get_kernel_time. */
 enum { FVNL_OPT_KERNEL = 0, FVNL_OPT_ROWS_PER_BLOCK = 1, FVNL_OPT_KERNEL_TIMING = 2, FVNL_OPT_VARIANT = 3 };
@@ -156,13 +159,14 @@ int fvnl_set_option(fvnl_ctx* ctx, int option, int value);
 enum { FVNL_TIMED_STEP = 0, FVNL_TIMED_XSWEEP = 1, FVNL_TIMED_YSWEEP = 2, FVNL_TIMED_SOURCE = 3, FVNL_TIMED_KINDS = 4 };
 int fvnl_get_kernel_time(fvnl_ctx* ctx, int which, double* total_ms, long* launches);
 
-/* FP64-pipe probe for the roofline denominator: runs a register-only kernel of independent DFMA chains (16 warps per
- * SM, 8 chains per thread) on the current device and stream and returns the achieved rate in TFLOP/s (FMA = 2 flop),
- * best of three.  Needs no context.  Errors: FVNL_EARG, FVNL_ECUDA. */
-int fvnl_probe_fp64(void* cuda_stream, double* tflops);
-
-/* Number of kernels this context has launched so far (sweeps, pre-pass, packing); for bench accounting. */
+/* Number of kernels this context has launched so far (step kernels, pre-pass, clock, boundary); for bench accounting. */
 long fvnl_kernel_launches(const fvnl_ctx* ctx);
+
+/* ---- MEASUREMENT AID, not part of the method --------------------------------------------------------------------------
+ * FP64-pipe probe for the roofline denominator of bench.py: runs a register-only kernel of independent DFMA chains (16
+ * warps per SM, 8 chains per thread) on the current device and stream and returns the achieved rate in TFLOP/s (FMA = 2
+ * flop), best of three.  Needs no context, touches no state.  Errors: FVNL_EARG, FVNL_ECUDA. */
+int fvnl_probe_fp64(void* cuda_stream, double* tflops);
 
 /* Text for a status code or flag word (static storage). */
 const char* fvnl_strerror(int code);

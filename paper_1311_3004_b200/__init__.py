@@ -54,10 +54,7 @@ def lib():
     """Load libfvnl.so (built in-tree by paper_1311_3004_b200.build; a missing compiler or library is an error)."""
     global _lib
     if _lib is None:
-        path = _build.LIB
-        if not os.path.exists(path) or os.environ.get("FVNL_REBUILD"):
-            path = _build.build()
-        L = C.CDLL(path)
+        L = C.CDLL(_build.build(force=bool(os.environ.get("FVNL_REBUILD"))))   # mtime-gated: never a stale binary
         L.fvnl_workspace_bytes.restype = C.c_size_t
         L.fvnl_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int]
         L.fvnl_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(fvnl_medium),

@@ -1,7 +1,9 @@
 // fvnl.cu -- C-ABI library of the B200-native finite-volume step of arXiv 1311.3004 (include/fvnl.h).
 //
-// Host side: context, argument checks, launch sequence.  All arithmetic of the path runs in the kernels of
-// fvnl_fused.cuh (default) or fvnl_unfused.cuh (opt-in comparison path); there is no CPU fallback.
+// Host side: context, argument checks, launch sequence.  All arithmetic of the path runs in the kernels: the
+// warp-specialised one-pass step kernel of fvnl_ws.cuh (default), the single-role one-pass kernel of fvnl_fused.cuh and the
+// three-pass kernels of fvnl_unfused.cuh (opt-in comparison paths), the clock / pre-pass / boundary kernels below; there is
+// no CPU fallback.
 // Build: paper_1311_3004_b200/build.py (nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo).
 #include <cstdio>
 #include <cstring>
@@ -14,75 +16,81 @@
 using namespace fvnl;
 
 // ---------------------------------------------------------------------------------------------------------------
-// Clock kernels (one thread).  PAPER.md:275-279, readings A7, A8.
-// mode 0: value = dt; mode 1: value = nu_W, dt = nu_W / (c0 M_prev).
-__global__ void k_clock_begin(Grid g, Clock* c, double value, int mode) {
-    const double dt = (mode == 1) ? __ddiv_rn(value, __dmul_rn(g.c0, c->Mprev)) : value;
-    c->dt = dt;
-    c->lamx = __ddiv_rn(__dmul_rn(g.c0, dt), g.dx);
-    c->lamy = __ddiv_rn(__dmul_rn(g.c0, dt), g.dy);
-    c->kapx = __ddiv_rn(__dmul_rn(g.delta, dt), __dmul_rn(g.dx, g.dx));
-    c->kapy = __ddiv_rn(__dmul_rn(g.delta, dt), __dmul_rn(g.dy, g.dy));
-    if (__dadd_rn(c->kapx, c->kapy) > 0.5) c->flags |= F_ECFL;
-    if (!(dt > 0.0) || not_finite(dt)) c->flags |= F_ENAN;
-    c->sx_bits = 0ull;
-    c->sy_bits = 0ull;
+// Clock kernels (one thread).  PAPER.md:275-279, readings A7, A8.  The end of a step (M_n, nu_n, t += dt and
+// the next dt) is NOT a kernel: the block of the step kernel that finishes last does it (step_tail, fvnl_fused.cuh).
+
+// fvnl_set_state: sticky flags and the lagged maximum are reset, t and the step counter stay.
+__global__ void k_clock_reset(Clock* c) {
+    c->flags = 0;
+    c->Mprev = 0.0;
+    c->sx_bits = c->sy_bits = 0ull;
+    c->ticket = 0u;
 }
 
-// End of step n (M_n, nu_n, t) fused with the beginning of step n+1 when `more` is set.
-__global__ void k_clock_end(Grid g, Clock* c, double value, int mode, int more) {
-    const double sx = __longlong_as_double((long long)c->sx_bits), sy = __longlong_as_double((long long)c->sy_bits);
-    const double M = fmax(__ddiv_rn(sx, g.dx), __ddiv_rn(sy, g.dy));
-    c->last_dt = c->dt;
-    c->last_cfl = __dmul_rn(__dmul_rn(g.c0, c->dt), M);
-    if (c->last_cfl > 1.0) c->flags |= F_ECFL;
+// fvnl_set_clock.
+__global__ void k_clock_set(Clock* c, double t, double M) {
+    c->t = t;
     c->Mprev = M;
-    c->t = __dadd_rn(c->t, c->dt);
-    c->steps += 1;
-    if (more) {
-        const double dt = (mode == 1) ? __ddiv_rn(value, __dmul_rn(g.c0, M)) : value;
-        c->dt = dt;
-        c->lamx = __ddiv_rn(__dmul_rn(g.c0, dt), g.dx);
-        c->lamy = __ddiv_rn(__dmul_rn(g.c0, dt), g.dy);
-        c->kapx = __ddiv_rn(__dmul_rn(g.delta, dt), __dmul_rn(g.dx, g.dx));
-        c->kapy = __ddiv_rn(__dmul_rn(g.delta, dt), __dmul_rn(g.dy, g.dy));
-        if (__dadd_rn(c->kapx, c->kapy) > 0.5) c->flags |= F_ECFL;
-        if (!(dt > 0.0) || not_finite(dt)) c->flags |= F_ENAN;
-        c->sx_bits = 0ull;
-        c->sy_bits = 0ull;
-    }
+    c->sx_bits = c->sy_bits = 0ull;
+    c->ticket = 0u;
 }
 
-// O7 pre-pass: M of the current state = max |s|/h over the x-interfaces of G_x(Q) and the y-interfaces of G_y(Q)
-// that touch an interior cell (first step of CFL mode).  Thread (i, j) owns its low interfaces (+ the high ones on
-// the last column / row).
-__global__ void __launch_bounds__(256) k_prepass(Grid g, Clock* clk, const double* __restrict__ q1,
-                                                 const double* __restrict__ q2, const double* __restrict__ q3) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y;
-    const double t = clk->t, b2 = 2.0 * (g.beta - 1.0);
-    int flags = 0;
-    double sx = 0.0, sy = 0.0;
-    if (i < g.nx) {
-        const Q3 c = load_ext(g, q1, q2, q3, i, j, t);
-        const CellX cx = make_cell(c.q1, c.q2, c.q3, flags), cy = make_cell(c.q1, c.q3, c.q2, flags);
-        {
-            const Q3 w = load_ext(g, q1, q2, q3, i - 1, j, t);
-            sx = max_speed(riemann_x(make_cell(w.q1, w.q2, w.q3, flags), cx, b2, flags));
-            if (i == g.nx - 1) {
-                const Q3 e = load_ext(g, q1, q2, q3, i + 1, j, t);
-                sx = fmax(sx, max_speed(riemann_x(cx, make_cell(e.q1, e.q2, e.q3, flags), b2, flags)));
-            }
-        }
-        {
-            const Q3 s = load_ext(g, q1, q2, q3, i, j - 1, t);
-            sy = max_speed(riemann_x(make_cell(s.q1, s.q3, s.q2, flags), cy, b2, flags));
-            if (j == g.ny - 1) {
-                const Q3 n = load_ext(g, q1, q2, q3, i, j + 1, t);
-                sy = fmax(sy, max_speed(riemann_x(cy, make_cell(n.q1, n.q3, n.q2, flags), b2, flags)));
-            }
-        }
+// Start of a fvnl_step call.  from_prepass: M_{n-1} is what k_prepass has just left in sx_bits / sy_bits.
+// mode 0: value = dt; mode 1: value = nu_W, dt = nu_W / (c0 M_prev).
+__global__ void k_clock_begin(Grid g, Clock* c, double value, int mode, int from_prepass) {
+    if (from_prepass) {
+        const double sx = __longlong_as_double((long long)c->sx_bits), sy = __longlong_as_double((long long)c->sy_bits);
+        c->Mprev = fmax(__ddiv_rn(sx, g.dx), __ddiv_rn(sy, g.dy));
     }
+    clock_set_dt(g, c, value, mode, c->Mprev);
+}
+
+// End of a step for the three-pass comparison path (its kernels have no tail).
+__global__ void k_clock_end(Grid g, Clock* c, double value, int mode, int more) { clock_advance(g, c, value, mode, more); }
+
+// The speed that enters M at one interface: max_p |s^p| = |v| + a of (32)-(34), which depends on the
+// density and the NORMAL velocity of the two cells only (z = q2/q1 for an x-interface, q3/q1 for a y-interface).
+__device__ __forceinline__ double iface_speed(double q1L, double zL, double q1R, double zR, double b2, double omb2, int& min_dhi) {
+    const double Zb1 = 0.5 * (q1L + q1R), Zb2 = 0.5 * (zL + zR);
+    const double v = Zb2 * rcp_o1(Zb1);
+    const double disc = fma(v, fma(-2.0, Zb2, v), fma(b2, Zb1, omb2));
+    min_dhi = min(min_dhi, hi_word(disc));
+    return fabs(v) + disc * rsqrt_o1(disc);
+}
+
+// O7 pre-pass: M of the current state = max |s|/h over the x-interfaces of G_x(Q) and the y-interfaces of G_y(Q) that
+// touch an interior cell (first step of CFL mode).  A read-only pass at HBM rate: every warp marches down a chunk of
+// PRE_ROWS rows over 32 consecutive columns (31 new ones + the left neighbour, handed over by shuffle -- no shared memory,
+// no barrier), the row below is carried in registers; analytic ghost cells come from k_sources' buffer.
+// grid = (ceil((nx + 1) / 124), ceil(ny / PRE_ROWS)), block = 128.
+constexpr int PRE_ROWS = 64;
+__global__ void __launch_bounds__(128) k_prepass(Grid g, Clock* clk, const double* __restrict__ q1,
+                                                 const double* __restrict__ q2, const double* __restrict__ q3) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int i_raw = ((int)blockIdx.x * 4 + warp) * 31 + lane - 1;           // column on the ghost-extended mesh, from -1
+    const int i = min(i_raw, g.nx);                                           // (lanes beyond the mesh idle on column nx)
+    const int j0 = (int)blockIdx.y * PRE_ROWS, j1 = min(j0 + PRE_ROWS, g.ny);
+    const int rlast = j1 == g.ny ? g.ny : j1 - 1;                             // the top chunk also owns interface ny - 1/2 + 1
+    const bool x_if = lane >= 1 && i_raw <= g.nx;                             // x-interface i - 1/2, i = 0 .. nx
+    const bool y_col = lane >= 1 && i_raw < g.nx;                             // y-interfaces of an interior column
+    const ColMap cm = map_column(g, i);
+    const double* src = src_buffer(g, clk->steps);
+    const double b2 = 2.0 * (g.beta - 1.0), omb2 = 1.0 - b2;
+    double sx = 0.0, sy = 0.0, below_q1 = 1.0, below_z3 = 0.0;
+    int mq = 0x7fffffff, md = 0x7fffffff;
+#pragma unroll 4
+    for (int r = j0 - 1; r <= rlast; ++r) {
+        const Q3 c = load_mapped(g, src, cm, i, r, q1, q2, q3);
+        mq = min(mq, hi_word(c.q1));
+        const double rc = rcp_o1(c.q1), z2 = c.q2 * rc, z3 = c.q3 * rc;
+        const double left_q1 = __shfl_up_sync(0xffffffffu, c.q1, 1), left_z2 = __shfl_up_sync(0xffffffffu, z2, 1);
+        if (x_if && r >= j0 && r < g.ny) sx = fmax(sx, iface_speed(left_q1, left_z2, c.q1, z2, b2, omb2, md));
+        if (y_col && r >= j0) sy = fmax(sy, iface_speed(below_q1, below_z3, c.q1, z3, b2, omb2, md));
+        below_q1 = c.q1; below_z3 = z3;
+    }
+    int flags = 0;
+    if (i_raw <= g.nx && mq <= 0) flags |= F_ENONPOS;
+    if (md < 0) flags |= F_ENONREAL;
     block_max_to(&clk->sx_bits, sx);
     __syncthreads();
     block_max_to(&clk->sy_bits, sy);
@@ -91,41 +99,13 @@ __global__ void __launch_bounds__(256) k_prepass(Grid g, Clock* clk, const doubl
 
 // Boundary / source-injection kernel: the analytic ghost cells (41), (43a-d), piston of every SOURCE side at t_n
 // (readings A11, A13, A14, A16), three layers deep, into Grid::src.  One thread per record.
-__global__ void __launch_bounds__(128) k_sources(Grid g, const Clock* clk, double* __restrict__ out) {
-    const double t = clk->t;
-    size_t n = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
-    for (int sd = 0; sd < 4; ++sd) {
-        const size_t recs = src_side_doubles(g.nx, g.ny, sd) / 3;
-        if (n < recs) {
-            if (g.side[sd].kind != BC_SOURCE) return;
-            const int per = sd < 2 ? g.ny + 6 : g.nx;
-            const int l = (int)(n / per), m = (int)(n % per);
-            Q3 c;
-            bool in;
-            if (sd < 2) {
-                const int r = m - 3, i = sd == SIDE_XLO ? -1 - l : g.nx + l;
-                in = source_cell(g.side[sd], sd, g.c0, (r + 0.5) * g.dy, (i + 0.5) * g.dx, t, c);
-            } else {
-                const double x = (m + 0.5) * g.dx;
-                in = source_cell(g.side[sd], sd, g.c0, x, x, t, c);
-            }
-            double* o = out + src_off(g.nx, g.ny, sd) + 3 * n;
-            o[0] = in ? c.q1 : -1.0; o[1] = in ? c.q2 : 0.0; o[2] = in ? c.q3 : 0.0;
-            return;
-        }
-        n -= recs;
-    }
+__global__ void __launch_bounds__(128) k_sources(Grid g, const Clock* clk) {
+    const size_t n = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    if (n < src_off(g.nx, g.ny, 4) / 3) source_record(g, clk->t, n, src_buffer(g, clk->steps));
 }
 
 __global__ void k_fill(double* p, size_t n, double v) {
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = v;
-}
-
-__global__ void k_prepass_end(Grid g, Clock* c) {
-    const double sx = __longlong_as_double((long long)c->sx_bits), sy = __longlong_as_double((long long)c->sy_bits);
-    c->Mprev = fmax(__ddiv_rn(sx, g.dx), __ddiv_rn(sy, g.dy));
-    c->sx_bits = 0ull;
-    c->sy_bits = 0ull;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -137,7 +117,7 @@ struct fvnl_ctx {
     void* ws;                   // workspace base
     bool own_ws;
     Clock* clk;                 // device clock
-    double* src;                // analytic ghost cells of the current step (k_sources)
+    double* src;                // analytic ghost cells of SOURCE sides, two buffers (src_buffer)
     double* buf[2][3];          // two state buffers (ping-pong); cur = index of the current state
     int cur;
     double* star[3];            // unfused path only: Q* on the y-extended mesh, allocated on first use
@@ -164,8 +144,9 @@ struct fvnl_ctx {
 };
 
 static const size_t MAX_SPANS = 1 << 16;
-static const int N_FUSED_VARIANTS = 4;
-static const int DEFAULT_VARIANT = 0;       // k_step_ws<96, 160>     // launch variants of the fused kernel (launch_fused)
+static const int N_FUSED_VARIANTS = 2;      // 0: k_step_ws (default), 1: k_step_fused
+static const int DEFAULT_VARIANT = 0;
+static const int FUSED_BX = 128, FUSED_MINB = 3;     // k_step_fused: block width, blocks per SM of its register budget
 
 // Event pair around one kernel launch (timing on only).
 struct SpanGuard {
@@ -202,7 +183,7 @@ static const size_t CLOCK_BYTES = 256;
 extern "C" size_t fvnl_workspace_bytes(int nx, int ny, int precision) {
     if (nx < 4 || ny < 4 || precision != 64) return 0;
     const size_t plane = align_up((size_t)nx * ny * sizeof(double), 256);
-    return CLOCK_BYTES + 6 * plane + align_up(src_off(nx, ny, 4) * sizeof(double), 256);
+    return CLOCK_BYTES + 6 * plane + align_up(2 * src_stride(nx, ny) * sizeof(double), 256);
 }
 
 #define CK(call)                                         \
@@ -264,6 +245,10 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
     c->need_prepass = true;
     c->kernel = FVNL_KERNEL_DEFAULT;
     c->variant = DEFAULT_VARIANT;
+    // per device (function attributes belong to the context of the current device)
+    ok = ok && cudaFuncSetAttribute(k_step_ws, cudaFuncAttributeMaxDynamicSharedMemorySize, ws_smem_bytes()) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(k_step_fused<FUSED_BX, FUSED_MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    fused_smem_bytes<FUSED_BX>()) == cudaSuccess;
     if (!ok) { (void)cudaGetLastError(); fvnl_destroy(c); return FVNL_ECUDA; }
     *out = c;
     return FVNL_OK;
@@ -330,14 +315,13 @@ extern "C" int fvnl_set_state(fvnl_ctx* c, const void* q1, const void* q2, const
     const void* src[3] = {q1, q2, q3};
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(c->buf[c->cur][k], src[k], c->n * sizeof(double), kind, c->stream));
-    // reset sticky flags and the lagged maximum, keep t (and the step counter)
+    // reset sticky flags and the lagged maximum, keep t (and the step counter): on the device, in stream order
+    k_clock_reset<<<1, 1, 0, c->stream>>>(c->clk);
+    c->launches += 1;
     c->snap.flags = 0;
     c->snap.Mprev = 0.0;
-    c->snap.sx_bits = c->snap.sy_bits = 0ull;
-    *c->host_clk = c->snap;
-    CK(cudaMemcpyAsync(c->clk, c->host_clk, sizeof(Clock), cudaMemcpyHostToDevice, c->stream));
-    if (!on_device) CK(cudaStreamSynchronize(c->stream));
-    else CK(cudaStreamSynchronize(c->stream));   // host_clk staging buffer is reused by later calls
+    if (!on_device) CK(cudaStreamSynchronize(c->stream));          // the host buffers may be reused on return
+    CK(cudaGetLastError());
     c->have_state = true;
     c->need_prepass = true;
     return FVNL_OK;
@@ -345,12 +329,12 @@ extern "C" int fvnl_set_state(fvnl_ctx* c, const void* q1, const void* q2, const
 
 extern "C" int fvnl_set_clock(fvnl_ctx* c, double t_s, double last_M) {
     if (!c || !(t_s == t_s)) return FVNL_EARG;
-    CK(cudaStreamSynchronize(c->stream));
+    const double M = last_M > 0.0 ? last_M : 0.0;
+    k_clock_set<<<1, 1, 0, c->stream>>>(c->clk, t_s, M);
+    c->launches += 1;
+    CK(cudaGetLastError());
     c->snap.t = t_s;
-    c->snap.Mprev = last_M > 0.0 ? last_M : 0.0;
-    *c->host_clk = c->snap;
-    CK(cudaMemcpyAsync(c->clk, c->host_clk, sizeof(Clock), cudaMemcpyHostToDevice, c->stream));
-    CK(cudaStreamSynchronize(c->stream));
+    c->snap.Mprev = M;
     c->need_prepass = !(last_M > 0.0);
     return FVNL_OK;
 }
@@ -387,45 +371,21 @@ static int fused_rows(const fvnl_ctx* c, int strips, int slots, int fill = 7) {
     return best_rows;
 }
 
-template <int BX, int MINB>
-static void launch_fused_t(fvnl_ctx* c, double** a, double** b) {
+// value / mode / more: what the block that finishes last needs to end the step (step_tail).
+static void launch_step(fvnl_ctx* c, double** a, double** b, double value, int mode, int more) {
     const Grid& g = c->g;
-    const int strips = (g.nx + (BX - 6) - 1) / (BX - 6);
-    const int rows = fused_rows(c, strips, 148 * MINB);
-    const dim3 grd(strips, (g.ny + rows - 1) / rows);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_step_fused<BX, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, fused_smem_bytes<BX>());
-        attr_set = true;
-    }
     SpanGuard sp(c, FVNL_TIMED_STEP);
-    k_step_fused<BX, MINB><<<grd, BX, fused_smem_bytes<BX>(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
-}
-
-template <int XREGS, int YREGS>
-static void launch_ws_t(fvnl_ctx* c, double** a, double** b) {
-    const Grid& g = c->g;
-    const int strips = (g.nx + (WS_COLS - 6) - 1) / (WS_COLS - 6);
-    const int per_sm = 65536 / (128 * (XREGS + YREGS));
-    const int rows = fused_rows(c, strips, 148 * per_sm, 8);
-    const dim3 grd(strips, (g.ny + rows - 1) / rows);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_step_ws<XREGS, YREGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, ws_smem_bytes());
-        attr_set = true;
-    }
-    SpanGuard sp(c, FVNL_TIMED_STEP);
-    k_step_ws<XREGS, YREGS><<<grd, 256, ws_smem_bytes(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows);
-}
-
-static void launch_fused(fvnl_ctx* c, double** a, double** b) {
-    // variants: 0 = warp-specialised kernel (default), 1 = the same without register re-balancing, 2.. = k_step_fused
-    const int variant = c->variant;
-    switch (variant) {
-        case 0: launch_ws_t<96, 160>(c, a, b); break;
-        case 1: launch_ws_t<128, 128>(c, a, b); break;
-        case 3: launch_fused_t<256, 1>(c, a, b); break;
-        default: launch_fused_t<128, 3>(c, a, b); break;
+    if (c->variant == 0) {
+        const int strips = (g.nx + (WS_COLS - 6) - 1) / (WS_COLS - 6);
+        const int rows = fused_rows(c, strips, 148 * WS_BLOCKS_PER_SM, 8);
+        const dim3 grd(strips, (g.ny + rows - 1) / rows);
+        k_step_ws<<<grd, 256, ws_smem_bytes(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows, value, mode, more);
+    } else {
+        const int strips = (g.nx + (FUSED_BX - 6) - 1) / (FUSED_BX - 6);
+        const int rows = fused_rows(c, strips, 148 * FUSED_MINB);
+        const dim3 grd(strips, (g.ny + rows - 1) / rows);
+        k_step_fused<FUSED_BX, FUSED_MINB><<<grd, FUSED_BX, fused_smem_bytes<FUSED_BX>(), c->stream>>>(
+            g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows, value, mode, more);
     }
 }
 
@@ -438,20 +398,21 @@ static int read_clock(fvnl_ctx* c) {
 
 static const size_t GRAPH_MAX_CELLS = 1u << 18;      // below this a step is a few microseconds: launches dominate
 
-// One time step of the default path on c->stream: boundary kernel (if any edge is a SOURCE), step kernel, clock kernel.
-static void default_step(fvnl_ctx* c, bool has_src, double value, int mode, int more) {
-    const Grid& g = c->g;
+static void launch_sources(fvnl_ctx* c) {
+    const size_t recs = src_off(c->g.nx, c->g.ny, 4) / 3;
+    k_sources<<<(unsigned)((recs + 127) / 128), 128, 0, c->stream>>>(c->g, c->clk);
+    c->launches += 1;
+}
+
+// One time step of the one-pass path on c->stream: ONE launch.  The step kernel's blocks also write the analytic ghost
+// cells of the step that follows (into the other buffer), and the block that finishes last ends the step (clock); only
+// the first step of a call gets its ghost cells from k_sources (the clock may have been set by the host in between).
+static void onepass_step(fvnl_ctx* c, double value, int mode, int more) {
     double** a = c->buf[c->cur];
     double** b = c->buf[c->cur ^ 1];
-    if (has_src && c->variant <= 1) {                           // this step's analytic ghost cells, at t_n
-        const size_t recs = src_off(g.nx, g.ny, 4) / 3;
-        k_sources<<<(unsigned)((recs + 127) / 128), 128, 0, c->stream>>>(g, c->clk, c->src);
-        c->launches += 1;
-    }
-    launch_fused(c, a, b);
+    launch_step(c, a, b, value, mode, more);
     c->cur ^= 1;
-    k_clock_end<<<1, 1, 0, c->stream>>>(g, c->clk, value, mode, more);
-    c->launches += 2;
+    c->launches += 1;
 }
 
 extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
@@ -466,15 +427,16 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
     if (mode == 0 && g.delta * value / (g.dx * g.dx) + g.delta * value / (g.dy * g.dy) > 0.5) return FVNL_EARG;
     if (nsteps == 0) return c->snap.flags;
     cudaStream_t st = c->stream;
-    const dim3 blk(256), grd((g.nx + 255) / 256, g.ny);
-    if (mode == 1 && c->need_prepass) {
-        k_prepass<<<grd, blk, 0, st>>>(g, c->clk, c->buf[c->cur][0], c->buf[c->cur][1], c->buf[c->cur][2]);
-        k_prepass_end<<<1, 1, 0, st>>>(g, c->clk);
-        c->launches += 2;
-        c->need_prepass = false;
+    if (has_src) launch_sources(c);                                 // analytic ghost cells at t_n of the first step
+    const int pre = (mode == 1 && c->need_prepass) ? 1 : 0;
+    if (pre) {                                                      // O7: M of the current state (k_clock_reset / _set
+        const dim3 grd((g.nx + 1 + 123) / 124, (g.ny + PRE_ROWS - 1) / PRE_ROWS);      // left the running maxima at zero)
+        k_prepass<<<grd, 128, 0, st>>>(g, c->clk, c->buf[c->cur][0], c->buf[c->cur][1], c->buf[c->cur][2]);
+        c->launches += 1;
     }
-    k_clock_begin<<<1, 1, 0, st>>>(g, c->clk, value, mode);
+    k_clock_begin<<<1, 1, 0, st>>>(g, c->clk, value, mode, pre);
     c->launches += 1;
+    c->need_prepass = false;                                        // from here on M_{n-1} is the last step's (reading A7)
     if (c->kernel == FVNL_KERNEL_UNFUSED) {
         const int rc = ensure_star(c);
         if (rc) return rc;
@@ -493,7 +455,7 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
                 const cudaStream_t user = c->stream;
                 c->stream = c->gstream;
                 const long l0 = c->launches;
-                for (int half = 0; half < 2; ++half) default_step(c, has_src, value, mode, 1);
+                for (int half = 0; half < 2; ++half) onepass_step(c, value, mode, 1);
                 c->launches = l0;                               // nothing ran: the capture only records
                 c->stream = user;
                 if (cudaStreamEndCapture(c->gstream, &graph) == cudaSuccess && graph &&
@@ -506,33 +468,30 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
             (void)cudaGetLastError();
         }
         if (c->gvalid) {
-            const int per_step = (has_src && c->variant <= 1 ? 1 : 0) + 2;
             for (; n + 3 <= nsteps; n += 2) {
                 CK(cudaGraphLaunch(c->gexec, st));
-                c->launches += 2 * per_step;
+                c->launches += 2;
             }
         }
     }
     for (; n < nsteps; ++n) {
+        const int more = n + 1 < nsteps ? 1 : 0;
         if (c->kernel == FVNL_KERNEL_DEFAULT) {
-            default_step(c, has_src, value, mode, n + 1 < nsteps ? 1 : 0);
+            onepass_step(c, value, mode, more);
             continue;
         }
         double** a = c->buf[c->cur];
         double** b = c->buf[c->cur ^ 1];
-        {
-            const dim3 grdx((g.nx + 255) / 256, g.ny + 4);
-            { SpanGuard sp(c, FVNL_TIMED_XSWEEP);
-              k_xsweep_unfused<<<grdx, blk, 0, st>>>(g, c->clk, a[0], a[1], a[2], c->star[0], c->star[1], c->star[2]); }
-            { SpanGuard sp(c, FVNL_TIMED_YSWEEP);
-              k_ysweep_unfused<<<grd, blk, 0, st>>>(g, c->clk, c->star[0], c->star[1], c->star[2], b[0], b[1], b[2]); }
-            { SpanGuard sp(c, FVNL_TIMED_SOURCE);
-              k_source_unfused<<<grd, blk, 0, st>>>(g, c->clk, b[0], b[1], b[2], a[0], a[1], a[2]); }
-            c->launches += 3;
-            // result is back in `a`: cur unchanged
-        }
-        k_clock_end<<<1, 1, 0, st>>>(g, c->clk, value, mode, n + 1 < nsteps ? 1 : 0);
-        c->launches += 1;
+        const dim3 blk(256), grd((g.nx + 255) / 256, g.ny), grdx((g.nx + 255) / 256, g.ny + 4);
+        { SpanGuard sp(c, FVNL_TIMED_XSWEEP);
+          k_xsweep_unfused<<<grdx, blk, 0, st>>>(g, c->clk, a[0], a[1], a[2], c->star[0], c->star[1], c->star[2]); }
+        { SpanGuard sp(c, FVNL_TIMED_YSWEEP);
+          k_ysweep_unfused<<<grd, blk, 0, st>>>(g, c->clk, c->star[0], c->star[1], c->star[2], b[0], b[1], b[2]); }
+        { SpanGuard sp(c, FVNL_TIMED_SOURCE);
+          k_source_unfused<<<grd, blk, 0, st>>>(g, c->clk, b[0], b[1], b[2], a[0], a[1], a[2]); }
+        // result is back in `a`: cur unchanged
+        k_clock_end<<<1, 1, 0, st>>>(g, c->clk, value, mode, more);
+        c->launches += 4;
     }
     CK(cudaGetLastError());
     const int rc = read_clock(c);

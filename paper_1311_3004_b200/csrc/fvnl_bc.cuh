@@ -22,7 +22,7 @@ struct Grid {
     int nx, ny;
     double dx, dy, c0, beta, delta;
     Side side[4];
-    const double* src;          // analytic ghost cells of this step, written by k_sources (null: no SOURCE side)
+    double* src;                // analytic ghost cells of SOURCE sides: two buffers (below), null without a SOURCE side
 };
 
 // Layout of Grid::src (doubles): three ghost layers per SOURCE side, layer l = distance - 1 from the edge; a record is
@@ -34,6 +34,12 @@ __host__ __device__ inline size_t src_off(int nx, int ny, int side) {
     size_t o = 0;
     for (int s = 0; s < side; ++s) o += src_side_doubles(nx, ny, s);
     return o;
+}
+// Two such buffers, used alternately: step n reads buffer n & 1 (values at t_n) while its blocks already write buffer
+// (n + 1) & 1 with the values at t_{n+1} = t_n + dt_n, which is known when step n starts (dt is lagged).
+__host__ __device__ inline size_t src_stride(int nx, int ny) { return (src_off(nx, ny, 4) + 31) / 32 * 32; }
+__host__ __device__ inline double* src_buffer(const Grid& g, long long step) {
+    return g.src ? g.src + (size_t)(step & 1) * src_stride(g.nx, g.ny) : nullptr;
 }
 
 // Device-resident clock: the time step lives here so that no host synchronisation is needed between steps
@@ -48,51 +54,117 @@ struct Clock {
     unsigned long long sx_bits, sy_bits;   // running max of |s| in x / y interfaces of the current step (bit patterns)
     long long steps;
     int flags;
-    int pad;
+    unsigned int ticket;        // blocks of the running step kernel that have finished (the last one ends the step)
 };
+
+// dt of the step about to start and everything derived from it.  mode 0: value = dt; mode 1: value = nu_W and
+// dt = nu_W / (c0 M), M = max |s|/h of the previous step (reading A7).  Also clears the running maxima.
+__device__ __forceinline__ void clock_set_dt(const Grid& g, Clock* c, double value, int mode, double M) {
+    const double dt = (mode == 1) ? __ddiv_rn(value, __dmul_rn(g.c0, M)) : value;
+    c->dt = dt;
+    c->lamx = __ddiv_rn(__dmul_rn(g.c0, dt), g.dx);
+    c->lamy = __ddiv_rn(__dmul_rn(g.c0, dt), g.dy);
+    c->kapx = __ddiv_rn(__dmul_rn(g.delta, dt), __dmul_rn(g.dx, g.dx));
+    c->kapy = __ddiv_rn(__dmul_rn(g.delta, dt), __dmul_rn(g.dy, g.dy));
+    if (__dadd_rn(c->kapx, c->kapy) > 0.5) c->flags |= F_ECFL;
+    if (!(dt > 0.0) || not_finite(dt)) c->flags |= F_ENAN;
+    c->sx_bits = 0ull;
+    c->sy_bits = 0ull;
+    c->ticket = 0u;
+}
+
+// End of step n: M_n from the running maxima, nu_n, t_{n+1}; and, when another step of the same call follows, its dt.
+__device__ __forceinline__ void clock_advance(const Grid& g, Clock* c, double value, int mode, int more) {
+    const double sx = __longlong_as_double((long long)*(volatile unsigned long long*)&c->sx_bits);
+    const double sy = __longlong_as_double((long long)*(volatile unsigned long long*)&c->sy_bits);
+    const double M = fmax(__ddiv_rn(sx, g.dx), __ddiv_rn(sy, g.dy));
+    c->last_dt = c->dt;
+    c->last_cfl = __dmul_rn(__dmul_rn(g.c0, c->dt), M);
+    if (c->last_cfl > 1.0) c->flags |= F_ECFL;
+    c->Mprev = M;
+    c->t = __dadd_rn(c->t, c->dt);
+    c->steps += 1;
+    c->ticket = 0u;
+    if (more) clock_set_dt(g, c, value, mode, M);
+}
 
 struct Q3 {
     double q1, q2, q3;
 };
 
-// Analytic boundary cell.  side: the edge the ghost cell belongs to; along: coordinate of its centre along that
-// edge from the low corner [m]; xc: x of its own centre from the x-lo edge [m] (TANH only).  Returns false when
-// the cell is outside the aperture (it then behaves as EXTRAP).
+// Analytic boundary cell: the value an edge of kind SOURCE prescribes for one of its ghost cells at time t.
+//   side   the edge the ghost cell belongs to;
+//   along  coordinate of the cell's centre along that edge, from the low corner [m];
+//   xc     x of the cell's own centre, from the x-lo edge [m] (used by the travelling profile (41) only).
+// Returns false for a cell outside the aperture: it then follows the extrapolation rule.
+//
+// (41), PAPER.md:330 (reading A11): the travelling profile q1 = 1 - K tanh(k (x - c0 t')), q2 = q1 - 1, q3 = 0.
+//
+// (43a-d), written from the geometry the paper describes rather than from its component formulas:
+// the transducer is a circular arc centred on the focus; the focus lies at distance F from the edge on the inward normal
+// through the centre of the aperture.  Seen from the edge point at signed distance x2 from that centre, the focus is in
+// the direction  F n - x2 e  (n: inward normal, e: along the edge), at distance hypot(F, x2).  The arc emits towards the
+// focus, so the momentum is g times the unit vector of that direction and the density is 1 + g; the point fires ahead of
+// the centre by the extra path, in the paraxial form the paper gives:  phase = f t' + x2^2 / (2 F lambda)  [periods].
+// g = A sin(2 pi phase) (piston, switched on at phase 0) or the same carrier under the packet envelope exp(-(phase/4)^10)
+// (reading A13).  F <= 0 or infinite: plane wave, direction n, no phase lead.
 __device__ __noinline__ bool source_cell(const Side& s, int side, double c0, double along, double xc, double t, Q3& out) {
-    if (s.shape == SRC_TANH) {                                            // (41), reading A11
-        const double q1 = 1.0 - s.amp * tanh(s.steep * (xc - c0 * (t + s.t0_s)));
-        out.q1 = q1; out.q2 = q1 - 1.0; out.q3 = 0.0;
+    const double tp = t + s.t0_s;
+    if (s.shape == SRC_TANH) {
+        const double rho1 = -s.amp * tanh(s.steep * fma(-c0, tp, xc));                // q1 - 1
+        out.q1 = 1.0 + rho1; out.q2 = out.q1 - 1.0; out.q3 = 0.0;
         return true;
     }
-    const double d = along - s.centre_m;                                   // x2 of (43)
-    if (s.half_aperture_m > 0.0 && fabs(d) > s.half_aperture_m) return false;
-    const bool focused = (s.focus_m > 0.0) && isfinite(s.focus_m);
-    double tau = s.freq_hz * (t + s.t0_s);                                 // periods
-    double cth = 1.0, sth = 0.0;
-    if (focused) {
-        const double lambda_w = c0 / s.freq_hz;
-        tau += d * d / (2.0 * s.focus_m * lambda_w);                       // tau = t + x2^2/(2F)
-        const double R = sqrt(d * d + s.focus_m * s.focus_m);
-        cth = s.focus_m / R;                                               // (43b)
-        sth = d / R;                                                       // (43c)
+    const double x2 = along - s.centre_m;
+    if (s.half_aperture_m > 0.0 && fabs(x2) > s.half_aperture_m) return false;
+    double phase = s.freq_hz * tp;
+    double to_focus_n = 1.0, to_focus_e = 0.0;                                        // unit vector towards the focus
+    if (s.focus_m > 0.0 && s.focus_m <= 1.7976931348623157e308) {
+        const double inv_dist = rhypot(s.focus_m, x2);
+        to_focus_n = s.focus_m * inv_dist;
+        to_focus_e = -x2 * inv_dist;
+        phase += (x2 / s.focus_m) * (x2 * s.freq_hz / c0) * 0.5;                      // x2^2/(2 F lambda), lambda = c0/f
     }
-    double g;
-    if (s.shape == SRC_SINE) {
-        g = (tau >= 0.0) ? s.amp * sin(2.0 * 3.14159265358979323846 * tau) : 0.0;
-    } else {                                                               // (43d) with reading A13
-        const double e = tau / 4.0;
-        const double e2 = e * e, e4 = e2 * e2, e8 = e4 * e4;
-        g = s.amp * sin(2.0 * 3.14159265358979323846 * tau) * exp(-(e8 * e2));
+    double g = s.amp * sinpi(2.0 * phase);
+    if (s.shape == SRC_PACKET) {
+        const double w = 0.25 * phase, w2 = w * w, w5 = w2 * w2 * w;
+        g *= exp(-(w5 * w5));
+    } else if (phase < 0.0) {
+        g = 0.0;
     }
-    const double qn = g * cth, qt = -g * sth;
-    out.q1 = 1.0 + g;                                                      // (43a)
-    switch (side) {
-        case SIDE_XLO: out.q2 = qn;  out.q3 = qt; break;
-        case SIDE_XHI: out.q2 = -qn; out.q3 = qt; break;
-        case SIDE_YLO: out.q3 = qn;  out.q2 = qt; break;
-        default:       out.q3 = -qn; out.q2 = qt; break;
-    }
+    const double m_n = (side & 1) ? -g * to_focus_n : g * to_focus_n;                 // hi sides: the inward normal is -x / -y
+    const double m_e = g * to_focus_e;
+    out.q1 = 1.0 + g;
+    if (side < 2) { out.q2 = m_n; out.q3 = m_e; }                                     // x sides: normal = x
+    else          { out.q2 = m_e; out.q3 = m_n; }                                     // y sides: normal = y
     return true;
+}
+
+// Record n of Grid::src (layout above): the analytic cell of one ghost position at time t; q1 = -1 marks "outside the
+// aperture".  n < src_off(nx, ny, 4) / 3.
+__device__ __forceinline__ void source_record(const Grid& g, double t, size_t n, double* __restrict__ out) {
+    size_t m = n;
+    for (int sd = 0; sd < 4; ++sd) {
+        const size_t recs = src_side_doubles(g.nx, g.ny, sd) / 3;
+        if (m < recs) {
+            if (g.side[sd].kind != BC_SOURCE) return;
+            const int per = sd < 2 ? g.ny + 6 : g.nx;
+            const int layer = (int)(m / per), pos = (int)(m % per);
+            Q3 c;
+            bool in;
+            if (sd < 2) {
+                const int r = pos - 3, i = sd == SIDE_XLO ? -1 - layer : g.nx + layer;
+                in = source_cell(g.side[sd], sd, g.c0, (r + 0.5) * g.dy, (i + 0.5) * g.dx, t, c);
+            } else {
+                const double x = (pos + 0.5) * g.dx;
+                in = source_cell(g.side[sd], sd, g.c0, x, x, t, c);
+            }
+            double* o = out + 3 * n;
+            o[0] = in ? c.q1 : -1.0; o[1] = in ? c.q2 : 0.0; o[2] = in ? c.q3 : 0.0;
+            return;
+        }
+        m -= recs;
+    }
 }
 
 __device__ __forceinline__ int wrap(int i, int n) {

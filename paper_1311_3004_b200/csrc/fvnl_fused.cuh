@@ -22,7 +22,7 @@
 // neighbouring interior Q** at the edge columns / rows.
 #pragma once
 #include "fvnl_unfused.cuh"
-#include "fvnl_pair.cuh"
+#include "fvnl_iface.cuh"
 
 namespace fvnl {
 
@@ -64,6 +64,52 @@ __device__ __forceinline__ RowMap map_row(const Grid& g, int r) {
         else { m.row = clampi(r, g.ny); if (kind == BC_SOURCE) m.ysrc = sd; }
     }
     return m;
+}
+
+// Cell (i, r) of the ghost-extended mesh, cm = map_column(g, i): the x rule first, then the y rule (reading A9: a corner
+// is the x-ghost of a y-ghost row); analytic cells of SOURCE sides from the buffer `src` of this step (src_buffer), where
+// a record with q1 <= 0 means "outside the aperture: extrapolate".
+__device__ __forceinline__ Q3 load_mapped(const Grid& g, const double* __restrict__ src, const ColMap& cm, int i, int r,
+                                          const double* __restrict__ q1, const double* __restrict__ q2,
+                                          const double* __restrict__ q3) {
+    const RowMap rm = map_row(g, r);
+    const size_t idx = (size_t)rm.row * g.nx + cm.col;
+    Q3 c;
+    c.q1 = q1[idx];
+    c.q2 = cm.neg2 ? -q2[idx] : q2[idx];
+    c.q3 = rm.neg3 ? -q3[idx] : q3[idx];
+    if (cm.xsrc >= 0 && r >= -3 && r <= g.ny + 2) {
+        const int l = cm.xsrc == SIDE_XLO ? -1 - i : i - g.nx;
+        if (l < 3) {
+            const double* sp = src + src_off(g.nx, g.ny, cm.xsrc) + 3 * ((size_t)(g.ny + 6) * l + r + 3);
+            if (sp[0] > 0.0) { c.q1 = sp[0]; c.q2 = sp[1]; c.q3 = sp[2]; return c; }
+        }
+    }
+    if (rm.ysrc >= 0) {
+        const int l = rm.ysrc == SIDE_YLO ? -1 - r : r - g.ny;
+        if (l < 3) {
+            const double* sp = src + src_off(g.nx, g.ny, rm.ysrc) + 3 * ((size_t)g.nx * l + cm.col);
+            if (sp[0] > 0.0) { c.q1 = sp[0]; c.q2 = cm.neg2 ? -sp[1] : sp[1]; c.q3 = sp[2]; }
+        }
+    }
+    return c;
+}
+
+// End of a step kernel: the running maxima and flags of this block are in the clock; the block that finishes last
+// advances the clock (clock_advance) -- no separate clock kernel, no host round trip (PAPER.md:279 lags dt by one step).
+// Every thread of the block must call it.
+__device__ __forceinline__ bool step_tail(const Grid& g, Clock* clk, double value, int mode, int more) {
+    __shared__ int is_last;
+    __threadfence();                                                // this thread's atomics before the ticket
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned total = gridDim.x * gridDim.y * gridDim.z;
+        is_last = atomicAdd(&clk->ticket, 1u) == total - 1u;
+        __threadfence();
+    }
+    __syncthreads();
+    if (is_last && threadIdx.x == 0) clock_advance(g, clk, value, mode, more);
+    return is_last;                                                 // block-uniform
 }
 
 // Analytic override of a loaded ghost value (same precedence as load_ext: x rule first, then y rule).  Rare path:
@@ -135,6 +181,7 @@ struct StepK {
     int j0, j1;                              // rows of output of this chunk: [j0, j1)
     int ylo, ycnt;                           // y-interface ry-1/2 is one the scheme solves iff (unsigned)(ry-ylo) <= ycnt
     bool px, py, any_src, any_refl;
+    const double* src;                       // analytic ghost cells of this step (k_step_ws), see src_buffer
 };
 
 // Per-thread constants and running reductions.
@@ -307,7 +354,7 @@ __global__ void __launch_bounds__(BX) __maxnreg__((65536 / (BX * MINB)) / 8 * 8 
 k_step_fused(Grid g, Clock* clk, const double* __restrict__ q1,
                                                          const double* __restrict__ q2, const double* __restrict__ q3,
                                                          double* __restrict__ o1, double* __restrict__ o2,
-                                                         double* __restrict__ o3, int rows) {
+                                                         double* __restrict__ o3, int rows, double value, int mode, int more) {
     extern __shared__ __align__(16) char smem[];
     const int tid = threadIdx.x;
     for (int k = tid; k < fused_smem_bytes<BX>() / 8; k += BX) reinterpret_cast<double*>(smem)[k] = 0.0;
@@ -387,6 +434,7 @@ k_step_fused(Grid g, Clock* clk, const double* __restrict__ q1,
     __syncthreads();
     block_max_to(&clk->sy_bits, y_col ? th.smy : 0.0);
     block_flags_to(&clk->flags, flags);
+    step_tail(g, clk, value, mode, more);
 }
 
 }  // namespace fvnl

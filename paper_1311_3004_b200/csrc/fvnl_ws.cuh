@@ -74,14 +74,14 @@ __device__ __forceinline__ void ws_xtick(const Grid& g, const StepK& k, XThread&
         if ((th.special & 8) && r >= -3 && r <= g.ny + 2) {
             const int sd = th.cm.xsrc, l = sd == SIDE_XLO ? -1 - th.i : th.i - g.nx;
             if (l < 3) {
-                const double* sp = g.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)(g.ny + 6) * l + r + 3);
+                const double* sp = k.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)(g.ny + 6) * l + r + 3);
                 if (sp[0] > 0.0) { a1 = sp[0]; a2 = sp[1]; a3 = sp[2]; done = true; }
             }
         }
         if (!STEADY && !done && rm.ysrc >= 0) {
             const int sd = rm.ysrc, l = sd == SIDE_YLO ? -1 - r : r - g.ny;
             if (l < 3) {
-                const double* sp = g.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)g.nx * l + th.cm.col);
+                const double* sp = k.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)g.nx * l + th.cm.col);
                 if (sp[0] > 0.0) { a1 = sp[0]; a2 = th.cm.neg2 ? -sp[1] : sp[1]; a3 = sp[2]; }
             }
         }
@@ -125,11 +125,12 @@ __device__ __forceinline__ void ws_xtick(const Grid& g, const StepK& k, XThread&
 // z of the one-deep ghost of Q** at a non-periodic edge, from the z of the interior cell next to it (reading A9): EXTRAP
 // copies, REFLECT negates the normal velocity, SOURCE takes the analytic cell of layer 0 (record `m`: the row for an x
 // side, the column for a y side) if it lies inside the aperture.
-__device__ __forceinline__ double2 ghost_z_plain(const Grid& g, int sd, int m, double z2, double z3) {
+__device__ __forceinline__ double2 ghost_z_plain(const Grid& g, const double* __restrict__ src, int sd, int m, double z2, double z3) {
     const int kind = g.side[sd].kind;
     if (kind == BC_REFLECT) return sd < 2 ? make_double2(-z2, z3) : make_double2(z2, -z3);
     if (kind == BC_SOURCE) {
-        const double* sp = g.src + src_off(g.nx, g.ny, sd) + 3 * (size_t)(sd < 2 ? m + 3 : m);
+        m = sd < 2 ? min(max(m, -3), g.ny + 2) : min(max(m, 0), g.nx - 1);          // (halo threads / pipeline fill: value unused)
+        const double* sp = src + src_off(g.nx, g.ny, sd) + 3 * (size_t)(sd < 2 ? m + 3 : m);
         if (sp[0] > 0.0) {
             const double rc = rcp_o1(sp[0]);
             return make_double2(sp[1] * rc, sp[2] * rc);
@@ -177,8 +178,8 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
     cy.q1 = N.c.q1; cy.q2 = N.c.q2; cy.q3 = N.c.q3;                           // Q*(ry-2), y-form: next tick's lower row
     double2 zW = lds2(p + ws_arr2(11, R) - 16), zE = lds2(p + ws_arr2(11, R) + 16);   // z of row ry-4, published last tick
     if (th.special & 3) {
-        if (th.special & 1) zW = ghost_z_plain(g, SIDE_XLO, ry - 4, cy.zC2, cy.zC3);
-        if (th.special & 2) zE = ghost_z_plain(g, SIDE_XHI, ry - 4, cy.zC2, cy.zC3);
+        if (th.special & 1) zW = ghost_z_plain(g, k.src, SIDE_XLO, ry - 4, cy.zC2, cy.zC3);
+        if (th.special & 2) zE = ghost_z_plain(g, k.src, SIDE_XHI, ry - 4, cy.zC2, cy.zC3);
     }
     const double H2 = fma(k.k2, cy.zC2, fma(k.kapx, zE.x + zW.x, cy.c2));
     const double H3 = fma(k.k2, cy.zC3, fma(k.kapx, zE.y + zW.y, cy.c3));
@@ -190,8 +191,8 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
         double y2 = zN2 + cy.zS2, y3 = zN3 + cy.zS3;
         if (!STEADY && !k.py && (Ro == 0 || Ro == g.ny - 1)) {
             double2 lo = make_double2(cy.zS2, cy.zS3), hi = make_double2(zN2, zN3);
-            if (Ro == 0) lo = ghost_z_plain(g, SIDE_YLO, th.i, cy.zC2, cy.zC3);
-            if (Ro == g.ny - 1) hi = ghost_z_plain(g, SIDE_YHI, th.i, cy.zC2, cy.zC3);
+            if (Ro == 0) lo = ghost_z_plain(g, k.src, SIDE_YLO, th.i, cy.zC2, cy.zC3);
+            if (Ro == g.ny - 1) hi = ghost_z_plain(g, k.src, SIDE_YHI, th.i, cy.zC2, cy.zC3);
             y2 = hi.x + lo.x; y3 = hi.y + lo.y;
         }
         const double w2 = fma(k.kapy, y2, H2), w3 = fma(k.kapy, y3, H3);
@@ -231,13 +232,13 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
 }
 
 // The step kernel.  grid = (strips, chunks); block = 256 threads (warps 0-3: X group, warps 4-7: Y group);
-// dynamic shared memory = ws_smem_bytes().  XREGS / YREGS: register budgets of the two groups (setmaxnreg); the
-// kernel is launched with their mean.
-template <int XREGS, int YREGS>
-__global__ void __launch_bounds__(256, 65536 / (128 * (XREGS + YREGS)))
+// dynamic shared memory = ws_smem_bytes().  The kernel is compiled for 128 registers per thread (2 blocks per SM) and
+// setmaxnreg moves registers from the X warps (96) to the Y warps (160).  value / mode / more: see step_tail.
+constexpr int WS_BLOCKS_PER_SM = 2;
+__global__ void __launch_bounds__(256, WS_BLOCKS_PER_SM)
 k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __restrict__ q2,
           const double* __restrict__ q3, double* __restrict__ o1, double* __restrict__ o2, double* __restrict__ o3,
-          int rows) {
+          int rows, double value, int mode, int more) {
     extern __shared__ __align__(16) char smem[];
     const int tid = threadIdx.x;
     for (int j = tid; j < ws_smem_bytes() / 8; j += 256) reinterpret_cast<double*>(smem)[j] = 1.0;   // finite fill
@@ -250,6 +251,8 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
     k.ylo = max(k.j0 - 2, -1); k.ycnt = g.ny + 1 - k.ylo;
     k.px = g.side[SIDE_XLO].kind == BC_PERIODIC; k.py = g.side[SIDE_YLO].kind == BC_PERIODIC;
     k.any_src = false; k.any_refl = false;
+    const long long step_no = clk->steps;
+    k.src = src_buffer(g, step_no);
     const int c = tid & (WS_COLS - 1);                             // column of the strip
     const int i = (int)blockIdx.x * (WS_COLS - 6) - 3 + c;         // column on the ghost-extended mesh
     const int r0 = k.j0 - 3, rend = k.j1 + 5;                      // the Y group runs behind, output row = r - 5
@@ -259,9 +262,7 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
 
     if (tid < WS_COLS) {
         // ================================= X group: the x-sweep =======================================================
-        if constexpr (XREGS == 96) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
-        if constexpr (XREGS == 104) asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
-        if constexpr (XREGS == 88) asm volatile("setmaxnreg.dec.sync.aligned.u32 88;");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
         XThread th;
         th.i = i;
         th.cm = map_column(g, i);
@@ -299,9 +300,7 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
         if (x_if_m) smx = th.smx;
     } else {
         // ================================= Y group: the y-sweep and the source step ===================================
-        if constexpr (YREGS == 160) asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
-        if constexpr (YREGS == 152) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
-        if constexpr (YREGS == 168) asm volatile("setmaxnreg.inc.sync.aligned.u32 168;");
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
         YThread th;
         th.i = i;
         th.special = (!k.px && i == 0 ? 1 : 0) | (!k.px && i == g.nx - 1 ? 2 : 0);
@@ -338,12 +337,23 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
         if (th.mxo >= 0x7ff00000) flags |= F_ENAN;
         if (y_col) smy = th.smy;
     }
+    // ---- analytic ghost cells of the NEXT step, t_{n+1} = t_n + dt_n (known since this step began), into the other buffer:
+    // every block's Y warps (the larger register budget) take a slice of the records
+    if (k.src && more && tid >= WS_COLS) {
+        const double t_next = __dadd_rn(k.t, clk->dt);
+        double* out = src_buffer(g, step_no + 1);
+        const size_t recs = src_off(g.nx, g.ny, 4) / 3, nblk = (size_t)gridDim.x * gridDim.y;
+        for (size_t n = ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * WS_COLS + (tid - WS_COLS); n < recs; n += nblk * WS_COLS)
+            source_record(g, t_next, n, out);
+    }
     // ---- reductions: M of and the sticky flags ---------------------------------------------------------
     __syncthreads();
     block_max_to(&clk->sx_bits, smx);
     __syncthreads();
     block_max_to(&clk->sy_bits, smy);
     block_flags_to(&clk->flags, flags);
+    // ---- the block that finishes last ends the step (clock) ----------------------------------------------------------
+    step_tail(g, clk, value, mode, more);
 }
 
 }  // namespace fvnl

@@ -203,3 +203,60 @@ def test_focused_field_is_mirror_symmetric_about_the_axis(focused_cw_run):
     assert np.abs(q2 - q2[::-1]).max() <= 1e-12 * amp
     assert np.abs(q3 + q3[::-1]).max() <= 1e-12 * amp
     assert np.abs(q3).max() > 0.2 * amp
+
+
+def _load_c4_script():
+    import importlib.util
+    import os
+    spec = importlib.util.spec_from_file_location(
+        "make_c4_windows", os.path.join(os.path.dirname(__file__), "golden", "make_c4_windows.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod
+
+
+def test_c4_golden_script_round_trip(tmp_path):
+    """tests/golden/make_c4_windows.py on a scaled-down C4: what it writes is, bit for bit, what the oracle holds (hex
+    floats), so neither the script nor the file format can go stale; the stored statistics are those of the state."""
+    mod = _load_c4_script()
+    w = W.c4_hifu(nx=160, ny=96, steps=60, focus_cells=60.0, aperture_cells=30.0, tau0=-1.0)
+    lines = mod.run(w, (20, 60), 6, 0)
+    path = tmp_path / "c4_small.txt"
+    path.write_text(mod.HEADER + "\n".join(lines) + "\n")
+    gold = mod.read(str(path))
+    assert gold["config"]["steps"] == [20, 60] and gold["config"]["win"] == 6
+    o = Oracle(w.nx, w.ny, w.dx, w.dy, **w.medium, threads=0)
+    o.set_bc(XLO, SOURCE, w.bc[0][1])
+    assert o.step(20, w.value, 1) == 0 and o.step(40, w.value, 1) == 0
+    q = o.get_state()
+    cp = gold["checkpoints"][60]
+    assert cp["t"] == o.info()["t"] and cp["M"] == o.info()["M"]
+    assert set(cp["windows"]) == {"edge_axis", "edge_half_aperture", "focus", "peak_q1", "peak_q3"}
+    for wd in cp["windows"].values():
+        for m in range(3):
+            assert np.array_equal(wd["q"][m], q[m][wd["j0"]:wd["j0"] + 6, wd["i0"]:wd["i0"] + 6])
+    assert cp["stats"][0]["max"] == np.abs(q[0] - 1.0).max() and cp["stats"][2]["l1"] == np.abs(q[2]).sum()
+
+
+def test_c4_golden_file_is_the_full_config():
+    """The stored file (when present) is C4 of BASELINE.json at full size and full step count, and what it holds is a
+    focused packet: nothing on the aperture at t = 0 ... the field at the focus exceeds the source amplitude (focusing
+    gain), the source edge is silent again once the packet has left, q3 is odd about the axis."""
+    import os
+    mod = _load_c4_script()
+    if not os.path.exists(mod.OUT):
+        pytest.skip("tests/golden/c4_full_windows.txt not generated yet")
+    gold = mod.read()
+    w = W.c4_hifu()
+    cfg = gold["config"]
+    assert (cfg["nx"], cfg["ny"], cfg["nu_w"], cfg["steps"][-1]) == (8192, 2048, 0.8, 4000) == (w.nx, w.ny, w.value, w.steps)
+    amp = w.bc[0][1]["amp"]
+    cps = gold["checkpoints"]
+    for cp in cps.values():
+        assert abs(cp["cfl"] - 0.8) < 2.5e-4 * 4                       # paper: std of nu <= 2.5e-4 on HIFU (PAPER.md:432)
+    assert 0.9 * amp < cps[400]["stats"][0]["max"] < 1.5 * amp          # packet being emitted
+    assert cps[3000]["stats"][0]["max"] > 2.0 * amp                     # at the focus (step ~2925): focusing gain
+    assert np.abs(cps[4000]["windows"]["edge_axis"]["q"][0] - 1.0).max() < 1e-3 * amp
+    ax = cps[3000]["windows"]["focus"]                                  # window centred on the axis: rows j0 .. j0+19
+    assert ax["j0"] + 10 == w.ny // 2
+    assert np.abs(ax["q"][2] + ax["q"][2][::-1]).max() <= 1e-9 * np.abs(ax["q"][2]).max()
