@@ -377,7 +377,7 @@ static void launch_step(fvnl_ctx* c, double** a, double** b, double value, int m
     SpanGuard sp(c, FVNL_TIMED_STEP);
     if (c->variant == 0) {
         const int strips = (g.nx + (WS_COLS - 6) - 1) / (WS_COLS - 6);
-        const int rows = fused_rows(c, strips, 148 * WS_BLOCKS_PER_SM, 8);
+        const int rows = fused_rows(c, strips, 148 * WS_BLOCKS_PER_SM, 9);
         const dim3 grd(strips, (g.ny + rows - 1) / rows);
         k_step_ws<<<grd, 256, ws_smem_bytes(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows, value, mode, more);
     } else {

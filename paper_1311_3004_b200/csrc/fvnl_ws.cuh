@@ -24,12 +24,12 @@
 namespace fvnl {
 
 constexpr int WS_COLS = 128;                  // columns of a strip = threads of each group
-// shared memory (bytes): arrays of double2, WS_COLS + 2 elements each
-//   single-buffered (X group only):   0 (q1,q2)  1 (q3,hz2)  2 (hz3,-)  3 (al1,s1)  4 (r31,al3)  5 (al2,s2)  6 (r32,-)
-//   double-buffered by tick parity:   7 (m1,m2)  8 (m3,-)  9 (u1,u2)  10 (u3,-)  [X -> Y]     11 (z2,z3)  [Y -> Y]
-__host__ __device__ constexpr int ws_arr(int k) { return k * (WS_COLS + 2) * 16; }
-__host__ __device__ constexpr int ws_arr2(int k, int parity) { return ws_arr(7 + 2 * (k - 7) + parity); }
-__host__ __device__ constexpr int ws_ring_off() { return ws_arr(7 + 2 * 5); }
+// shared memory (bytes): arrays of double2, WS_COLS + 2 elements each, ALL double-buffered by the parity of the row they hold
+//   X group:  0 (q1,q2)  1 (q3,hz2)  2 (hz3,-)  [cells]      3 (al1,s1)  4 (r31,al3)  5 (al2,s2)  6 (r32,-)  [waves]
+//   X -> Y:   7 (m1,m2)  8 (m3,ft1)  9 (u1,u2)  10 (u3,p1)       Y -> Y:  11 (z2,z3)
+constexpr int WS_ARRAYS = 12;
+__host__ __device__ constexpr int ws_arr2(int k, int parity) { return (2 * k + parity) * (WS_COLS + 2) * 16; }
+__host__ __device__ constexpr int ws_ring_off() { return 2 * WS_ARRAYS * (WS_COLS + 2) * 16; }
 __host__ __device__ constexpr int ws_smem_bytes() { return ws_ring_off() + 4 * 3 * WS_COLS * 8; }
 
 __device__ __forceinline__ void bar_x() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
@@ -41,85 +41,113 @@ struct XThread {
     char *p, *pq;
     double smx;
     int mqx, mdx;
+    Wv w;                                    // waves of interface i-1/2 of the row solved in the previous tick
+    double rn1, rn2;                         // and their 1/(r.r)
+    Cx cx;                                   // this column's cell of the row converted in the previous tick
+    double aq[2][3];                         // Q^n(i, .) of the rows loaded in the previous two ticks, by row parity
 };
 
-// One tick of an X warp: the x-sweep of row r up to the two halves of the update (27).
+// One tick of an X warp.  The x-sweep is software-pipelined over rows: tick t runs three INDEPENDENT pieces of work, each on
+// its own row, so that the warp has several dependency chains to issue from (a dependent FP64 operation waits 9 cycles) and
+// ONE block-wide barrier per tick separates everything:
+//   phase C, row t   : limited fluxes (28)-(30) of interface i-1/2 from its waves (solved in tick t-1, kept in registers)
+//                      and the upwind neighbour's (shared memory) -> the two halves of the update (27) for the Y warps;
+//   phase B, row t+1 : Riemann solve between the cells of columns i-1 and i (converted in tick t-1)
+//                      -> waves to shared memory;
+//   phase A, row t+2 : Q^n(., t+2) from the prefetch ring, ghost rule, primitive conversion -> cell to shared memory;
+//                      prefetch of row t+4.
+// P = t & 1.  FILL: one of the two ticks before the Y warps start (the barrier is then the X group's own).
 template <int P, bool STEADY>
-__device__ __forceinline__ void ws_xtick(const Grid& g, const StepK& k, XThread& th, int r,
+__device__ __forceinline__ void ws_xtick(const Grid& g, const StepK& k, XThread& th, int t, int r0,
                                          const double* __restrict__ q1, const double* __restrict__ q2,
                                          const double* __restrict__ q3) {
     char* const p = th.p;
-    RowMap rm, rm_pre;                                                        // rows r and r+2 (the one to prefetch)
-    if (STEADY) {
-        rm.row = r; rm.neg3 = false; rm.ysrc = -1;
-        rm_pre.row = r + 2;
-    } else {
-        rm = map_row(g, r);
-        rm_pre = map_row(g, r + 2);
-    }
-    cp_async_wait<1>();                                                       // row r has landed
-    double a1, a2, a3;
-    {
-        const char* ps = th.pq + (r & 3) * (3 * WS_COLS * 8);
-        a1 = lds1(ps); a2 = lds1(ps + WS_COLS * 8); a3 = lds1(ps + 2 * WS_COLS * 8);
-        char* pd = th.pq + ((r + 2) & 3) * (3 * WS_COLS * 8);
-        const size_t idx = (size_t)rm_pre.row * g.nx + th.cm.col;
-        cp_async8(pd, q1 + idx); cp_async8(pd + WS_COLS * 8, q2 + idx); cp_async8(pd + 2 * WS_COLS * 8, q3 + idx);
-        cp_async_commit();
-    }
-    if ((th.special & 12) || (!STEADY && (rm.neg3 || rm.ysrc >= 0))) {        // ghost column / row with a rule: rare
-        if (!STEADY && rm.neg3) a3 = -a3;
-        if (th.special & 4) a2 = -a2;
-        bool done = false;                                                    // x rule first, then y rule (as load_ext)
-        if ((th.special & 8) && r >= -3 && r <= g.ny + 2) {
-            const int sd = th.cm.xsrc, l = sd == SIDE_XLO ? -1 - th.i : th.i - g.nx;
-            if (l < 3) {
-                const double* sp = k.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)(g.ny + 6) * l + r + 3);
-                if (sp[0] > 0.0) { a1 = sp[0]; a2 = sp[1]; a3 = sp[2]; done = true; }
-            }
-        }
-        if (!STEADY && !done && rm.ysrc >= 0) {
-            const int sd = rm.ysrc, l = sd == SIDE_YLO ? -1 - r : r - g.ny;
-            if (l < 3) {
-                const double* sp = k.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)g.nx * l + th.cm.col);
-                if (sp[0] > 0.0) { a1 = sp[0]; a2 = th.cm.neg2 ? -sp[1] : sp[1]; a3 = sp[2]; }
-            }
-        }
-    }
-    int tq = 0x7fffffff, td = 0x7fffffff;
-    const Cx cx = cell_of(a1, a2, a3, tq);
-    sts2(p + ws_arr(0), cx.q1, cx.q2); sts2(p + ws_arr(1), cx.q3, cx.hz2); sts1(p + ws_arr(2), cx.hz3);
-    bar_x();                                                                  // cells visible
-    Cx L;
-    {
-        const double2 u0 = lds2(p + ws_arr(0) - 16), u1 = lds2(p + ws_arr(1) - 16);
-        L.q1 = u0.x; L.q2 = u0.y; L.q3 = u1.x; L.hz2 = u1.y; L.hz3 = lds1(p + ws_arr(2) - 16);
-    }
-    const Wv w = riemann2(L, cx, k.b2, k.omb2, td);
-    const double rn1 = rnorm(w.s1, w.r31), rn2 = rnorm(w.s2, w.r32);
-    sts2(p + ws_arr(3), w.al1, w.s1); sts2(p + ws_arr(4), w.r31, w.al3); sts2(p + ws_arr(5), w.al2, w.s2);
-    sts1(p + ws_arr(6), w.r32);
-    if (STEADY || (unsigned)r < (unsigned)g.ny) {
-        th.mqx = min(th.mqx, tq); th.mdx = min(th.mdx, td);
-        th.smx = dmax(th.smx, fabs(hi_word(w.v) < 0 ? w.s2 : w.s1));          // max(|s1|,|s2|) = |v| + a
-    }
-    bar_x();                                                                  // waves visible
-    {
+    constexpr int Q = P ^ 1;
+    // ---- phase C: row t ----------------------------------------------------------------------------------------------
+    if (STEADY || t >= r0) {
+        const Wv& w = th.w;
         const char* u1 = p + (hi_word(w.s1) < 0 ? 16 : -16);                  // upwind interface
         const char* u2 = p + (hi_word(w.s2) < 0 ? 16 : -16);
         const char* u3 = p + (hi_word(w.v) < 0 ? 16 : -16);
-        const double2 k1 = lds2(u1 + ws_arr(3)), k2 = lds2(u2 + ws_arr(5));
-        const double k1r = lds1(u1 + ws_arr(4)), k2r = lds1(u2 + ws_arr(6)), k3 = lds1(u3 + ws_arr(4) + 8);
-        const double b1 = k1.x * rdot(k1.y, k1r, w.s1, w.r31) * rn1;
-        const double b2 = k2.x * rdot(k2.y, k2r, w.s2, w.r32) * rn2;
+        const double2 k1 = lds2(u1 + ws_arr2(3, P)), k2 = lds2(u2 + ws_arr2(5, P));
+        const double k1r = lds1(u1 + ws_arr2(4, P)), k2r = lds1(u2 + ws_arr2(6, P)), k3 = lds1(u3 + ws_arr2(4, P) + 8);
+        const double own1 = th.aq[P][0], own2 = th.aq[P][1], a3 = th.aq[P][2];   // Q^n(i, t), loaded two ticks ago
+        const double b1 = k1.x * rdot(k1.y, k1r, w.s1, w.r31) * th.rn1;
+        const double b2 = k2.x * rdot(k2.y, k2r, w.s2, w.r32) * th.rn2;
         const Fl F = flux2(w, b1, b2, k3, k.lamx);
-        // the two halves of (27) for row r: what this interface sends left, and this column's own part
+        // the two halves of (27) for row t: what this interface sends left, and this column's own part
         // (the density component goes over unrounded: q1, p1 and the first component of F~, see update_q1)
         sts2(p + ws_arr2(7, P), F.m1, F.m2); sts2(p + ws_arr2(8, P), F.m3, F.ft1);
-        sts2(p + ws_arr2(9, P), a1, fma(-k.lamx, F.p2, a2));
+        sts2(p + ws_arr2(9, P), own1, fma(-k.lamx, F.p2, own2));
         sts2(p + ws_arr2(10, P), fma(-k.lamx, F.p3, a3), F.p1);
     }
-    bar_all();                                                                // row r handed to the Y warps
+    // ---- phase B: row t+1 --------------------------------------------------------------------------------------------
+    if (STEADY || t + 1 >= r0) {
+        Cx L;
+        const Cx C = th.cx;
+        {
+            const double2 l0 = lds2(p + ws_arr2(0, Q) - 16), l1 = lds2(p + ws_arr2(1, Q) - 16);
+            L.q1 = l0.x; L.q2 = l0.y; L.q3 = l1.x; L.hz2 = l1.y; L.hz3 = lds1(p + ws_arr2(2, Q) - 16);
+        }
+        int td = 0x7fffffff;
+        const Wv w = riemann2(L, C, k.b2, k.omb2, td);
+        th.rn1 = rnorm(w.s1, w.r31); th.rn2 = rnorm(w.s2, w.r32);
+        th.w = w;
+        sts2(p + ws_arr2(3, Q), w.al1, w.s1); sts2(p + ws_arr2(4, Q), w.r31, w.al3); sts2(p + ws_arr2(5, Q), w.al2, w.s2);
+        sts1(p + ws_arr2(6, Q), w.r32);
+        if (STEADY || (unsigned)(t + 1) < (unsigned)g.ny) {
+            th.mdx = min(th.mdx, td);
+            th.smx = dmax(th.smx, fabs(hi_word(w.v) < 0 ? w.s2 : w.s1));      // max(|s1|,|s2|) = |v| + a
+        }
+    }
+    // ---- phase A: row t+2 (prefetch row t+4) -------------------------------------------------------------------------
+    {
+        const int r = t + 2;
+        RowMap rm, rm_pre;
+        if (STEADY) {
+            rm.row = r; rm.neg3 = false; rm.ysrc = -1;
+            rm_pre.row = r + 2;
+        } else {
+            rm = map_row(g, r);
+            rm_pre = map_row(g, r + 2);
+        }
+        cp_async_wait<1>();                                                   // row t+2 has landed
+        double a1, a2, a3;
+        {
+            const char* ps = th.pq + (r & 3) * (3 * WS_COLS * 8);
+            a1 = lds1(ps); a2 = lds1(ps + WS_COLS * 8); a3 = lds1(ps + 2 * WS_COLS * 8);
+            char* pd = th.pq + ((r + 2) & 3) * (3 * WS_COLS * 8);
+            const size_t idx = (size_t)rm_pre.row * g.nx + th.cm.col;
+            cp_async8(pd, q1 + idx); cp_async8(pd + WS_COLS * 8, q2 + idx); cp_async8(pd + 2 * WS_COLS * 8, q3 + idx);
+            cp_async_commit();
+        }
+        if ((th.special & 12) || (!STEADY && (rm.neg3 || rm.ysrc >= 0))) {    // ghost column / row with a rule: rare
+            if (!STEADY && rm.neg3) a3 = -a3;
+            if (th.special & 4) a2 = -a2;
+            bool done = false;                                                // x rule first, then y rule (as load_mapped)
+            if ((th.special & 8) && r >= -3 && r <= g.ny + 2) {
+                const int sd = th.cm.xsrc, l = sd == SIDE_XLO ? -1 - th.i : th.i - g.nx;
+                if (l < 3) {
+                    const double* sp = k.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)(g.ny + 6) * l + r + 3);
+                    if (sp[0] > 0.0) { a1 = sp[0]; a2 = sp[1]; a3 = sp[2]; done = true; }
+                }
+            }
+            if (!STEADY && !done && rm.ysrc >= 0) {
+                const int sd = rm.ysrc, l = sd == SIDE_YLO ? -1 - r : r - g.ny;
+                if (l < 3) {
+                    const double* sp = k.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)g.nx * l + th.cm.col);
+                    if (sp[0] > 0.0) { a1 = sp[0]; a2 = th.cm.neg2 ? -sp[1] : sp[1]; a3 = sp[2]; }
+                }
+            }
+        }
+        int tq = 0x7fffffff;
+        const Cx cx = cell_of(a1, a2, a3, tq);
+        sts2(p + ws_arr2(0, P), cx.q1, cx.q2); sts2(p + ws_arr2(1, P), cx.q3, cx.hz2); sts1(p + ws_arr2(2, P), cx.hz3);
+        th.cx = cx;
+        th.aq[P][0] = a1; th.aq[P][1] = a2; th.aq[P][2] = a3;
+        if (STEADY || (unsigned)r < (unsigned)g.ny) th.mqx = min(th.mqx, tq);
+    }
+    if (!STEADY && t < r0) bar_x(); else bar_all();                           // the Y warps join at tick r0
 }
 
 // z of the one-deep ghost of Q** at a non-periodic edge, from the z of the interior cell next to it (reading A9): EXTRAP
@@ -148,18 +176,22 @@ struct YThread {
 };
 
 struct YCarry {
-    double gp1, gp2, gp3, gf1;               // right-going part (and F~, comp. 1) of the y-interface below the newest one
-    double q1, q2, q3;                       // Q*(., ry-3), y-form
-    double c1, c2, c3, zC2, zC3;             // Q**(ry-4) and its z
-    double zS2, zS3;                         // z of Q**(ry-5)
+    double gp1, gp2, gp3, gf1;               // right-going part (and F~, comp. 1) of the y-interface below B
+    double q1, q2, q3;                       // Q*(., ry-4), y-form
+    double c1, c2, c3, zC2, zC3;             // Q**(ry-5) and its z
+    double zS2, zS3;                         // z of Q**(ry-6)
+    Cx pend;                                 // cell of Q*(., ry-1), y-form: converted in the previous tick, solved in this one
 };
 
-// One tick of a Y warp (tick r works on ry = r-1).  Two independent chains, so that the warp has two instructions to
-// choose from at every step:
-//   chain 1:  Q*(., ry) from what the X warps published in the previous tick -> cell -> y-Riemann solve at ry-1/2 (N)
-//             -> limiter inputs between N and the interface below it (A), which are now final for A;
-//   chain 2:  limited flux of the interface two below N (B, at ry-5/2: its limiter inputs became final in the previous
-//             tick) -> Q**(., ry-3) -> source step for row ry-4 -> Q^{n+1}(., ry-4) -> HBM.
+// One tick of a Y warp (tick r works on ry = r-1, the row the X warps published in the previous tick).  I(k) = the
+// y-interface between rows k-1 and k.  THREE independent chains per tick -- the y-sweep is software-pipelined over rows so
+// that the warp always has several instructions to choose from against the 9-cycle FP64 latency, and so that the longest
+// dependent chain of a tick is the Riemann solve alone:
+//   chain 1a:  Q*(., ry) completed from what the X warps published -> primitive conversion (cy.pend, solved next tick);
+//   chain 1b:  y-Riemann solve of N = I(ry-1) from the two cells converted in earlier ticks -> limiter inputs between N
+//              and A = I(ry-2), which are now final for A;
+//   chain 2:   limited flux of B = I(ry-3) (its limiter inputs became final in the previous tick) -> Q**(., ry-4)
+//              -> source step for row ry-5 -> Q^{n+1}(., ry-5) -> HBM.
 // P = r & 1: parity this tick publishes into (it reads parity P^1); Y[P] holds B on entry and N on exit, Y[P^1] is A.
 template <int P, bool STEADY>
 __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread& th, YCarry& cy, YSet& Y0, YSet& Y1, int r,
@@ -169,24 +201,24 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
     constexpr int R = P ^ 1;
     char* const p = th.p;
     const int ry = r - 1;
-    // ---- chain 2: flux of B, Q**(., ry-3), source step ----------------------------------------------------------------
+    // ---- chain 2: flux of B, Q**(., ry-4), source step ----------------------------------------------------------------
     const Fl G = flux2(N.w, N.pb1, N.pb2, N.pb3, k.lamy);                     // N still holds B
-    const double n1 = update_q1(cy.q1, k.lamy, cy.gp1 + G.m1, cy.gf1, G.ft1); // Q**(i, ry-3); physical order n1, n2, n3
+    const double n1 = update_q1(cy.q1, k.lamy, cy.gp1 + G.m1, cy.gf1, G.ft1); // Q**(i, ry-4); physical order n1, n2, n3
     const double n3 = fma(-k.lamy, cy.gp2 + G.m2, cy.q2);
     const double n2 = fma(-k.lamy, cy.gp3 + G.m3, cy.q3);
     cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3; cy.gf1 = G.ft1;
-    cy.q1 = N.c.q1; cy.q2 = N.c.q2; cy.q3 = N.c.q3;                           // Q*(ry-2), y-form: next tick's lower row
-    double2 zW = lds2(p + ws_arr2(11, R) - 16), zE = lds2(p + ws_arr2(11, R) + 16);   // z of row ry-4, published last tick
+    cy.q1 = N.c.q1; cy.q2 = N.c.q2; cy.q3 = N.c.q3;                           // Q*(ry-3), y-form: next tick's lower row
+    double2 zW = lds2(p + ws_arr2(11, R) - 16), zE = lds2(p + ws_arr2(11, R) + 16);   // z of row ry-5, published last tick
     if (th.special & 3) {
-        if (th.special & 1) zW = ghost_z_plain(g, k.src, SIDE_XLO, ry - 4, cy.zC2, cy.zC3);
-        if (th.special & 2) zE = ghost_z_plain(g, k.src, SIDE_XHI, ry - 4, cy.zC2, cy.zC3);
+        if (th.special & 1) zW = ghost_z_plain(g, k.src, SIDE_XLO, ry - 5, cy.zC2, cy.zC3);
+        if (th.special & 2) zE = ghost_z_plain(g, k.src, SIDE_XHI, ry - 5, cy.zC2, cy.zC3);
     }
     const double H2 = fma(k.k2, cy.zC2, fma(k.kapx, zE.x + zW.x, cy.c2));
     const double H3 = fma(k.k2, cy.zC3, fma(k.kapx, zE.y + zW.y, cy.c3));
     const double rq = rcp_o1(n1);
     const double zN2 = n2 * rq, zN3 = n3 * rq;
     sts2(p + ws_arr2(11, P), zN2, zN3);
-    const int Ro = ry - 4;
+    const int Ro = ry - 5;
     if (STEADY || Ro >= k.j0) {                                               // Ro < j1 by the loop bound
         double y2 = zN2 + cy.zS2, y3 = zN3 + cy.zS3;
         if (!STEADY && !k.py && (Ro == 0 || Ro == g.ny - 1)) {
@@ -205,17 +237,9 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
     cy.zS2 = cy.zC2; cy.zS3 = cy.zC3;
     cy.c1 = n1; cy.c2 = n2; cy.c3 = n3; cy.zC2 = zN2; cy.zC3 = zN3;
 
-    // ---- chain 1: Q*(., ry), interface ry-1/2 (N), final limiter inputs of A ---------------------------------------------
-    double s1, s2, s3;                                                        // Q*(i, ry): the update (27) completed
-    {
-        const double2 u = lds2(p + ws_arr2(9, R)), gm = lds2(p + ws_arr2(7, R) + 16);
-        const double2 u3 = lds2(p + ws_arr2(10, R)), gm3 = lds2(p + ws_arr2(8, R) + 16);
-        const double ft_own = lds1(p + ws_arr2(8, R) + 8);
-        s1 = update_q1(u.x, k.lamx, u3.y + gm.x, ft_own, gm3.y);
-        s2 = fma(-k.lamx, gm.y, u.y); s3 = fma(-k.lamx, gm3.x, u3.x);
-    }
-    int tqy = 0x7fffffff, tdy = 0x7fffffff;
-    N.c = cell_of(s1, s3, s2, tqy);                                           // positions 2,3 switched
+    // ---- chain 1b: interface N = I(ry-1) between the cells of Q*(ry-2) (A.c) and Q*(ry-1) (cy.pend); limiter inputs of A ----
+    int tdy = 0x7fffffff;
+    N.c = cy.pend;
     N.w = riemann2(A.c, N.c, k.b2, k.omb2, tdy);
     N.rn1 = rnorm(N.w.s1, N.w.r31); N.rn2 = rnorm(N.w.s2, N.w.r32);
     const double d1 = rdot(A.w.s1, A.w.r31, N.w.s1, N.w.r31), d2 = rdot(A.w.s2, A.w.r32, N.w.s2, N.w.r32);
@@ -224,9 +248,21 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepK& k, YThread&
     A.pb1 = hi_word(A.w.s1) < 0 ? hb1 : A.pb1;                                // A's upwind side is now known
     A.pb2 = hi_word(A.w.s2) < 0 ? hb2 : A.pb2;
     A.pb3 = hi_word(A.w.v) < 0 ? N.w.al3 : A.pb3;
-    if (STEADY || (unsigned)(ry - k.ylo) <= (unsigned)k.ycnt) {               // y-interface ry-1/2 is one the scheme solves
-        th.mqy = min(th.mqy, tqy); th.mdy = min(th.mdy, tdy);
-        if (STEADY || (unsigned)ry <= (unsigned)g.ny) th.smy = dmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
+    if (STEADY || (unsigned)(ry - 1 - k.ylo) <= (unsigned)k.ycnt) {           // I(ry-1) is an interface the scheme solves
+        th.mdy = min(th.mdy, tdy);
+        if (STEADY || (unsigned)(ry - 1) <= (unsigned)g.ny) th.smy = dmax(th.smy, fabs(hi_word(N.w.v) < 0 ? N.w.s2 : N.w.s1));
+    }
+
+    // ---- chain 1a: Q*(., ry), the update (27) completed, and its primitive conversion for the next tick ----------------
+    {
+        const double2 u = lds2(p + ws_arr2(9, R)), gm = lds2(p + ws_arr2(7, R) + 16);
+        const double2 u3 = lds2(p + ws_arr2(10, R)), gm3 = lds2(p + ws_arr2(8, R) + 16);
+        const double ft_own = lds1(p + ws_arr2(8, R) + 8);
+        const double s1 = update_q1(u.x, k.lamx, u3.y + gm.x, ft_own, gm3.y);
+        const double s2 = fma(-k.lamx, gm.y, u.y), s3 = fma(-k.lamx, gm3.x, u3.x);
+        int tqy = 0x7fffffff;
+        cy.pend = cell_of(s1, s3, s2, tqy);                                   // positions 2,3 switched
+        if (STEADY || (unsigned)(ry - k.ylo) <= (unsigned)k.ycnt) th.mqy = min(th.mqy, tqy);   // a cell the y-sweep uses
     }
     bar_all();
 }
@@ -255,7 +291,7 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
     k.src = src_buffer(g, step_no);
     const int c = tid & (WS_COLS - 1);                             // column of the strip
     const int i = (int)blockIdx.x * (WS_COLS - 6) - 3 + c;         // column on the ghost-extended mesh
-    const int r0 = k.j0 - 3, rend = k.j1 + 5;                      // the Y group runs behind, output row = r - 5
+    const int r0 = k.j0 - 3, rend = k.j1 + 6;                      // the Y group runs behind, output row = r - 6
     double smx = 0.0, smy = 0.0;
     int flags = 0;
     __syncthreads();                                               // (the fill above is complete)
@@ -270,6 +306,10 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
         th.p = smem + (c + 1) * 16;
         th.pq = smem + ws_ring_off() + c * 8;
         th.smx = 0.0; th.mqx = th.mdx = 0x7fffffff;
+        th.w = {0.0, 1.0, 0.0, 0.0, -1.0, 0.0, 0.0, 0.0};
+        th.rn1 = th.rn2 = 0.5;
+        th.cx = {1.0, 0.0, 0.0, 0.0, 0.0};
+        for (int d = 0; d < 2; ++d) th.aq[d][0] = 1.0, th.aq[d][1] = th.aq[d][2] = 0.0;
         for (int d = 0; d < 2; ++d) {                              // rows r0 and r0+1 start their way into the ring
             const RowMap rm = map_row(g, r0 + d);
             const size_t idx = (size_t)rm.row * g.nx + th.cm.col;
@@ -277,19 +317,19 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
             cp_async8(pd, q1 + idx); cp_async8(pd + WS_COLS * 8, q2 + idx); cp_async8(pd + 2 * WS_COLS * 8, q3 + idx);
             cp_async_commit();
         }
-        int r = r0;
-        const int slo = 0, shi = min(rend - 1, g.ny - 3);          // steady: rows r .. r+2 are interior rows
-        while (r < rend && (r < slo || (r & 1))) {
-            if (r & 1) ws_xtick<1, false>(g, k, th, r, q1, q2, q3); else ws_xtick<0, false>(g, k, th, r, q1, q2, q3);
-            ++r;
+        int t = r0 - 2;                                            // two ticks of pipeline fill before the Y warps start
+        const int slo = 0, shi = min(rend - 1, g.ny - 5);          // steady: rows t .. t+4 are interior rows, t >= r0
+        while (t < rend && (t < max(slo, r0) || (t & 1))) {
+            if (t & 1) ws_xtick<1, false>(g, k, th, t, r0, q1, q2, q3); else ws_xtick<0, false>(g, k, th, t, r0, q1, q2, q3);
+            ++t;
         }
-        for (; r + 1 <= shi; r += 2) {
-            ws_xtick<0, true>(g, k, th, r, q1, q2, q3);
-            ws_xtick<1, true>(g, k, th, r + 1, q1, q2, q3);
+        for (; t + 1 <= shi; t += 2) {
+            ws_xtick<0, true>(g, k, th, t, r0, q1, q2, q3);
+            ws_xtick<1, true>(g, k, th, t + 1, r0, q1, q2, q3);
         }
-        while (r < rend) {
-            if (r & 1) ws_xtick<1, false>(g, k, th, r, q1, q2, q3); else ws_xtick<0, false>(g, k, th, r, q1, q2, q3);
-            ++r;
+        while (t < rend) {
+            if (t & 1) ws_xtick<1, false>(g, k, th, t, r0, q1, q2, q3); else ws_xtick<0, false>(g, k, th, t, r0, q1, q2, q3);
+            ++t;
         }
         cp_async_wait<0>();
         const bool x_if_m = c >= 1 && i >= 0 && i <= g.nx;          // x-interface i-1/2 touches an interior cell
@@ -316,9 +356,10 @@ k_step_ws(Grid g, Clock* clk, const double* __restrict__ q1, const double* __res
         cy.gp1 = cy.gp2 = cy.gp3 = cy.gf1 = 0.0;
         cy.q1 = 1.0; cy.q2 = cy.q3 = 0.0;
         cy.c1 = 1.0; cy.c2 = cy.c3 = cy.zC2 = cy.zC3 = cy.zS2 = cy.zS3 = 0.0;
+        cy.pend = Y0.c;
         int r = r0;
-        // steady: interface ry-1/2 (ry = r-1) is a real one, output row r-5 >= j0 and away from the y edges
-        const int slo = max(k.j0 + 5, k.py ? 0 : 6), shi = min(rend - 1, g.ny);
+        // steady: the interface solved (I(ry-1), ry = r-1) is a real one, output row r-6 >= j0 and away from the y edges
+        const int slo = max(k.j0 + 6, k.py ? 0 : 7), shi = min(rend - 1, g.ny);
         while (r < rend && (r < slo || (r & 1))) {
             if (r & 1) ws_ytick<1, false>(g, k, th, cy, Y0, Y1, r, o1, o2, o3); else ws_ytick<0, false>(g, k, th, cy, Y0, Y1, r, o1, o2, o3);
             ++r;
