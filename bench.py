@@ -26,14 +26,24 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "fp64 Gcell-updates/s"
+METRIC = "fp64 Gcell-updates/s"          # (with --precision 32 the same quantity for the fp32 variant; `dtype` says which)
 UNIT = "Gcell-updates/s"
-ALG_BYTES_PER_CELL = 48.0          # 3 fields x 8 B x (1 read + 1 write) per cell-update
+ALG_BYTES_PER_VALUE = 6.0          # 3 fields x (1 read + 1 write) per cell-update, x 8 B (f64) or 4 B (f32)
 ALG_FLOP_PER_CELL = 404.0          # the oracle's formulas, division / sqrt = 1
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 lanes x FMA x 1965 MHz = 37.2
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel, from the committed `ncu --set full`
-# capture (profiles/r1_ws_ncu_summary.md): 6.590525 + 6.402814 GB at 16384^2, i.e. 48.4 B per cell-update
-NCU_TRAFFIC_BYTES = {"C5-16384": 12.993339e9}
+# derived ALU peaks (not in MEASURED_PEAKS.json): 148 SMs x lanes x FMA x 1965 MHz; 64 FP64 lanes, 128 FP32 lanes per SM
+ALU_PEAK_TFLOPS = {64: 148 * 64 * 2 * 1.965e9 / 1e12, 32: 148 * 128 * 2 * 1.965e9 / 1e12}
+
+
+def ncu_traffic(workload, precision):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel, from the committed `ncu --set full`
+    capture of THIS kernel on THIS workload (profiles/r2_traffic.json, which names the capture) -- None when there is none:
+    the figure is a property of a capture, it is not measured in the run."""
+    try:
+        d = json.load(open(os.path.join(ROOT, "profiles", "r2_traffic.json")))
+        e = d.get(f"{workload}/f{precision}")
+        return (float(e["dram_bytes_per_launch"]), e["capture"]) if e else (None, None)
+    except Exception:
+        return None, None
 
 
 def reduce_max_ms(ms, dist, device):
@@ -220,7 +230,7 @@ def run_gpu(args):
 
     w = make_workload(args.workload)
     K, Wm = args.steps, args.warmup
-    s = P.Solver(w.nx, w.ny, w.dx, w.dy, **w.medium, device=dev)
+    s = P.Solver(w.nx, w.ny, w.dx, w.dy, **w.medium, device=dev, precision=args.precision)
     for side, (kind, src) in enumerate(w.bc):
         s.set_bc(side, kind, src)
     if args.kernel == "unfused":
@@ -284,20 +294,24 @@ def run_gpu(args):
     top = max(spans, key=lambda k: spans[k][0])
     top_ms = spans[top][0] / spans[top][1]
     share = spans[top][0] / ms
+    traffic_src = "--traffic" if args.traffic is not None else None
     if args.traffic is None and args.kernel == "fused" and args.variant in (-1, 0):
-        args.traffic = NCU_TRAFFIC_BYTES.get(w.name)
-    achieved = ALG_BYTES_PER_CELL * w.cells / (top_ms * 1e-3) / 1e9
+        args.traffic, traffic_src = ncu_traffic(w.name, args.precision)
+    alg_bytes = ALG_BYTES_PER_VALUE * (args.precision // 8) * w.cells
+    achieved = alg_bytes / (top_ms * 1e-3) / 1e9
     roofline_hbm = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                    "frac": achieved / peak, "traffic": args.traffic, "peak_source": peak_src,
-                    "algorithmic_bytes_per_launch": ALG_BYTES_PER_CELL * w.cells}
+                    "frac": achieved / peak, "traffic": args.traffic, "traffic_source": traffic_src,
+                    "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes}
     rc_probe, probe_tflops = P.fvnl_probe_fp64(torch.cuda.current_stream(dev).cuda_stream)
     tf = ALG_FLOP_PER_CELL * w.cells / (top_ms * 1e-3) / 1e12
     sm_mhz = clocks.get("sm_mhz") or 1965.0
-    roofline = {"bound": "alu", "kernel": top, "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": tf / FP64_PEAK_TFLOPS, "traffic": args.traffic,
-                "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x 1.965 GHz (DESIGN.md 7); fp64 vector pipe, "
-                               "not in MEASURED_PEAKS.json",
-                "frac_at_observed_clock": tf / (FP64_PEAK_TFLOPS * sm_mhz / 1965.0),
+    alu_peak = ALU_PEAK_TFLOPS[args.precision]
+    lanes = 64 if args.precision == 64 else 128
+    roofline = {"bound": "alu", "kernel": top, "achieved": tf, "peak": alu_peak, "unit": "TFLOP/s",
+                "frac": tf / alu_peak, "traffic": args.traffic, "traffic_source": traffic_src,
+                "peak_source": f"derived: 148 SMs x {lanes} FP{args.precision} lanes x 2 flop x 1.965 GHz (DESIGN.md 7); "
+                               f"fp{args.precision} vector pipe, not in MEASURED_PEAKS.json",
+                "frac_at_observed_clock": tf / (alu_peak * sm_mhz / 1965.0),
                 "fp64_probe_tflops": probe_tflops if rc_probe == 0 else None,   # DFMA-only kernel, measured in this run
                 "algorithmic_flop_per_launch": ALG_FLOP_PER_CELL * w.cells, "ms_per_launch": top_ms,
                 "share_of_step": share,
@@ -334,12 +348,14 @@ def run_gpu(args):
     base = cpu_baseline(w) if not args.no_cpu else None
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
-        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": f"f{args.precision}",
         "data": "synthetic",
         "config": {"workload": w.name, "grid": [w.nx, w.ny], "cells": w.cells, "bc": [k for k, _ in w.bc],
                    "nu_W": w.value, "kernel": top if args.kernel == "fused" else "three-pass (" + top + " is the slowest of the three)",
-                   "variant": args.variant, "rows_per_block": args.rows, "state_bytes": 24 * w.cells,
-                   "l2": "state larger than L2, no flush" if 24 * w.cells > 4 * 126e6 else "state near/below L2 size",
+                   "variant": args.variant, "rows_per_block": args.rows, "state_bytes": 3 * (args.precision // 8) * w.cells,
+                   "precision": args.precision,
+                   "l2": "state larger than L2, no flush" if 3 * (args.precision // 8) * w.cells > 4 * 126e6 else "state near/below L2 size",
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "flags": int(flags),
                    "t_end_s": info["t"], "last_cfl": info["cfl"]},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_hbm": roofline_hbm,
@@ -364,6 +380,8 @@ def main():
     ap.add_argument("--variant", type=int, default=-1, help="launch variant of the fused kernel (tuning aid)")
     ap.add_argument("--rows", type=int, default=0, help="rows per block of the fused kernel (0 = automatic)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--precision", type=int, default=64, choices=[64, 32],
+                    help="64: the paper's precision and the metric's (default); 32: the single-precision variant (PAPER.md:464)")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
     args = ap.parse_args()

@@ -20,7 +20,7 @@
  *   - State = the paper's dimensionless conserved vector q of (22), PAPER.md:133:
  *         q1 = rho/rho0,  q2 = q1*u/c0,  q3 = q1*v/c0        (equilibrium: 1, 0, 0)
  *     as three separate contiguous planes of nx*ny values, index = j*nx + i, i = x index (fastest).
- *   - Pointers named `*_dev_or_host` are device pointers when `on_device != 0`, host pointers otherwise.
+ *   - Pointers named `*_dev_or_host` are device pointers when `where & FVNL_ON_DEVICE`, host pointers otherwise.
  *   - SI units at the boundary (m, s, Hz); only lambda = c0 dt/dx, kappa = delta dt/dx^2 and beta enter the update.
  */
 #ifndef FVNL_H
@@ -82,11 +82,17 @@ typedef struct {
     double steep;           /* TANH only                                                               */
 } fvnl_source;
 
-/* Bytes of device memory the context needs for an nx x ny grid (second state buffer, clock, reduction slots).
- * precision: 64 (fp32 is not built in this round -> 0 is returned for anything else). */
+/* Precision of a context.  64: the paper's, state planes of double holding q.  32: the single-precision
+ * variant ("sometimes ... as good", faster), PERTURBATION FORM: the state planes are float and hold
+ * (rho' = q1 - 1, q2, q3), so that fp32 round-off is relative to the acoustic perturbation and not to the unit background;
+ * all arithmetic of the step is fp32, the clock (t, dt, M) and the analytic boundary cells stay fp64.  Everything else
+ * (edges, sources, modes, flags) is the same; the comparison kernels (fvnl_set_option) exist in fp64 only.
+ *
+ * Bytes of device memory the context needs for an nx x ny grid (two states, clock, analytic ghost cells); 0 for bad
+ * arguments. */
 size_t fvnl_workspace_bytes(int nx, int ny, int precision);
 
-/* Create a context.  nx, ny >= 4; dx, dy, c0, rho0 > 0; beta >= 1; delta >= 0; precision = 64.
+/* Create a context.  nx, ny >= 4; dx, dy, c0, rho0 > 0; beta >= 1; delta >= 0; precision = 64 or 32.
  * cuda_stream: a cudaStream_t (NULL = default stream); all work of this context is issued on it.
  * workspace: DEVICE memory of at least fvnl_workspace_bytes() bytes, 256-byte aligned, owned by the caller (e.g. a
  * torch tensor) and kept alive until fvnl_destroy; or NULL, then the library cudaMallocs it itself.
@@ -102,12 +108,19 @@ void fvnl_destroy(fvnl_ctx* ctx);
  * missing src.  A lone PERIODIC side is reported by fvnl_step (FVNL_EARG). */
 int fvnl_set_bc(fvnl_ctx* ctx, int side, int kind, const fvnl_source* src_or_null);
 
-/* Copy a state in (three planes of nx*ny doubles).  Resets the sticky flags and the lagged maximum M (the next
+/* Where the planes passed to fvnl_set_state / fvnl_get_state live and what they hold (OR-ed):
+ *   FVNL_ON_DEVICE   device pointers (else host pointers);
+ *   FVNL_PLANES_F64  fp32 contexts only, device pointers only: the planes are double and hold the standard state q; the
+ *                    library converts to / from its stored form (rho', q2, q3) in a kernel.  Ignored by fp64 contexts.
+ * Without FVNL_PLANES_F64 the planes are in the context's own form: double q (precision 64), float (rho', q2, q3) (32). */
+enum { FVNL_ON_HOST = 0, FVNL_ON_DEVICE = 1, FVNL_PLANES_F64 = 2 };
+
+/* Copy a state in (three planes of nx*ny values, see above).  Resets the sticky flags and the lagged maximum M (the next
  * CFL-mode step starts with the pre-pass), keeps t.  Device input: asynchronous, everything (copies and the clock reset)
  * is queued on the stream and the call returns at once.  Host input: the call synchronises the stream, so the buffers may
  * be reused when it returns. */
 int fvnl_set_state(fvnl_ctx* ctx, const void* q1_dev_or_host, const void* q2_dev_or_host,
-                   const void* q3_dev_or_host, int on_device);
+                   const void* q3_dev_or_host, int where);
 
 /* Set the clock: simulation time t [s] and the lagged maximum M [1/m] of the previous step.
  * last_M <= 0: M unknown -- the next CFL-mode step recomputes it by the pre-pass on the state as it is then, unless a
@@ -129,8 +142,9 @@ int fvnl_set_clock(fvnl_ctx* ctx, double t_s, double last_M);
  * FVNL_ECUDA. */
 int fvnl_step(fvnl_ctx* ctx, long nsteps, double value, int mode);
 
-/* Copy the current state out (three planes of nx*ny doubles).  Synchronises the stream for host output. */
-int fvnl_get_state(fvnl_ctx* ctx, void* q1_dev_or_host, void* q2_dev_or_host, void* q3_dev_or_host, int on_device);
+/* Copy the current state out (three planes of nx*ny values, `where` as for fvnl_set_state).  Synchronises the stream for
+ * host output. */
+int fvnl_get_state(fvnl_ctx* ctx, void* q1_dev_or_host, void* q2_dev_or_host, void* q3_dev_or_host, int where);
 
 /* Clock and step statistics after the last fvnl_step: time [s], last dt [s], CFL number of the last step
  * nu = c0*dt*M, last M [1/m], number of steps taken since fvnl_create.  Any pointer may be NULL.  Synchronises. */

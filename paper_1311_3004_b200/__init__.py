@@ -28,6 +28,7 @@ ECFL, ENONREAL, ENONPOS, ENAN = 16, 32, 64, 128
 OPT_KERNEL, OPT_ROWS_PER_BLOCK, OPT_KERNEL_TIMING, OPT_VARIANT = 0, 1, 2, 3
 TIMED_STEP, TIMED_XSWEEP, TIMED_YSWEEP, TIMED_SOURCE = 0, 1, 2, 3
 KERNEL_DEFAULT, KERNEL_UNFUSED = 0, 1
+ON_HOST, ON_DEVICE, PLANES_F64 = 0, 1, 2
 
 
 class fvnl_medium(C.Structure):
@@ -102,8 +103,8 @@ def fvnl_set_option(h, option, value):
     return lib().fvnl_set_option(h, option, value)
 
 
-def fvnl_set_state(h, p1, p2, p3, on_device):
-    return lib().fvnl_set_state(h, _vp(p1), _vp(p2), _vp(p3), int(on_device))
+def fvnl_set_state(h, p1, p2, p3, where):
+    return lib().fvnl_set_state(h, _vp(p1), _vp(p2), _vp(p3), int(where))
 
 
 def fvnl_set_clock(h, t_s, last_M):
@@ -114,8 +115,8 @@ def fvnl_step(h, nsteps, value, mode):
     return lib().fvnl_step(h, int(nsteps), float(value), int(mode))
 
 
-def fvnl_get_state(h, p1, p2, p3, on_device):
-    return lib().fvnl_get_state(h, _vp(p1), _vp(p2), _vp(p3), int(on_device))
+def fvnl_get_state(h, p1, p2, p3, where):
+    return lib().fvnl_get_state(h, _vp(p1), _vp(p2), _vp(p3), int(where))
 
 
 def fvnl_get_info(h):
@@ -147,25 +148,31 @@ def fvnl_strerror(code):
 
 # ---- convenience object -----------------------------------------------------------------------------------------
 class Solver:
-    """One fvnl context on the current CUDA device and torch's current stream.  State tensors are (ny, nx) float64."""
+    """One fvnl context on the current CUDA device and torch's current stream.
 
-    def __init__(self, nx, ny, dx, dy, c0, rho0, beta, delta, device="cuda", stream=None):
+    precision 64: state tensors are (ny, nx) float64 holding q.  precision 32 (perturbation form, include/fvnl.h): the
+    context stores float32 planes (rho' = q1 - 1, q2, q3); set_state / get_state take either such float32 tensors, or
+    float64 tensors holding the standard q, which the LIBRARY converts on the device (FVNL_PLANES_F64)."""
+
+    def __init__(self, nx, ny, dx, dy, c0, rho0, beta, delta, device="cuda", stream=None, precision=64):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1311_3004_b200 needs a CUDA device; there is no CPU fallback")
         self.device = torch.device(device)
         if self.device.type != "cuda":
             raise RuntimeError("paper_1311_3004_b200 runs on CUDA devices only")
         self.nx, self.ny = int(nx), int(ny)
+        self.precision = int(precision)
+        self.dtype = torch.float64 if self.precision == 64 else torch.float32
         self._h = None
         with torch.cuda.device(self.device):
-            nbytes = fvnl_workspace_bytes(self.nx, self.ny, 64)
+            nbytes = fvnl_workspace_bytes(self.nx, self.ny, self.precision)
             if nbytes == 0:
                 raise FvnlError("fvnl_workspace_bytes", EARG)
             # torch owns the device memory; +256 so that a 256-byte aligned base always exists
             self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             base = (self._ws.data_ptr() + 255) // 256 * 256
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            rc, h = fvnl_create(self.nx, self.ny, dx, dy, fvnl_medium(c0, rho0, beta, delta), 64,
+            rc, h = fvnl_create(self.nx, self.ny, dx, dy, fvnl_medium(c0, rho0, beta, delta), self.precision,
                                 self._stream.cuda_stream, base, nbytes)
         if rc:
             raise FvnlError("fvnl_create", rc)
@@ -198,18 +205,24 @@ class Solver:
 
     def _prep(self, a):
         a = torch.as_tensor(a)
-        if a.dtype != torch.float64 or a.numel() != self.nx * self.ny:
-            raise ValueError("state planes must be float64 with nx*ny elements")
+        if a.dtype not in (torch.float64, self.dtype) or a.numel() != self.nx * self.ny:
+            raise ValueError("state planes must be float64 (q) or the context's own dtype, with nx*ny elements")
         return a.contiguous()
 
     def set_state(self, q1, q2, q3):
         """Copy a state in; CUDA tensors are read on the device, CPU tensors / arrays from host memory."""
         q = [self._prep(a) for a in (q1, q2, q3)]
         on_dev = q[0].is_cuda
-        if any(a.is_cuda != on_dev for a in q):
-            raise ValueError("all three planes must live on the same side")
+        if any(a.is_cuda != on_dev or a.dtype != q[0].dtype for a in q):
+            raise ValueError("all three planes must live on the same side and have one dtype")
+        where = ON_DEVICE if on_dev else ON_HOST
+        if self.precision == 32 and q[0].dtype == torch.float64:      # standard q for an fp32 context: the library converts,
+            q = [a.to(self.device) for a in q]                         # on the device (torch only moves the bytes there)
+            where = ON_DEVICE | PLANES_F64
         with torch.cuda.device(self.device):
-            self._check("fvnl_set_state", fvnl_set_state(self._h, q[0].data_ptr(), q[1].data_ptr(), q[2].data_ptr(), on_dev))
+            self._check("fvnl_set_state", fvnl_set_state(self._h, q[0].data_ptr(), q[1].data_ptr(), q[2].data_ptr(), where))
+            if where & PLANES_F64:
+                self._stream.synchronize()                             # the temporaries above are read asynchronously
 
     def set_clock(self, t, last_M=0.0):
         self._check("fvnl_set_clock", fvnl_set_clock(self._h, t, last_M))
@@ -222,17 +235,26 @@ class Solver:
             raise FvnlError("fvnl_step", rc)
         return rc
 
-    def get_state(self, out=None, host=False):
-        """Current state as three (ny, nx) tensors: on the device, or (host=True) in (pinned) host memory.
+    def get_state(self, out=None, host=False, as_q64=False):
+        """Current state as three (ny, nx) tensors in the context's own form: on the device, or (host=True) in (pinned)
+        host memory.  as_q64 (fp32 contexts): float64 device tensors holding the standard q, converted by the library.
         `out`: three preallocated tensors to fill instead."""
         if out is None:
-            if host:
-                out = [torch.empty(self.ny, self.nx, dtype=torch.float64, pin_memory=True) for _ in range(3)]
-            else:
+            if as_q64:
                 out = [torch.empty(self.ny, self.nx, dtype=torch.float64, device=self.device) for _ in range(3)]
-        on_dev = out[0].is_cuda
+            elif host:
+                out = [torch.empty(self.ny, self.nx, dtype=self.dtype, pin_memory=True) for _ in range(3)]
+            else:
+                out = [torch.empty(self.ny, self.nx, dtype=self.dtype, device=self.device) for _ in range(3)]
+        where = ON_DEVICE if out[0].is_cuda else ON_HOST
+        if self.precision == 32 and out[0].dtype == torch.float64:
+            if not out[0].is_cuda:
+                raise ValueError("float64 output of an fp32 context is produced on the device")
+            where |= PLANES_F64
+        elif out[0].dtype != self.dtype:
+            raise ValueError("output planes must have the context's dtype")
         with torch.cuda.device(self.device):
-            self._check("fvnl_get_state", fvnl_get_state(self._h, out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), on_dev))
+            self._check("fvnl_get_state", fvnl_get_state(self._h, out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), where))
         return out
 
     def info(self):

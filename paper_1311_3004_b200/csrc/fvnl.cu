@@ -64,8 +64,9 @@ __device__ __forceinline__ double iface_speed(double q1L, double zL, double q1R,
 // no barrier), the row below is carried in registers; analytic ghost cells come from k_sources' buffer.
 // grid = (ceil((nx + 1) / 124), ceil(ny / PRE_ROWS)), block = 128.
 constexpr int PRE_ROWS = 64;
-__global__ void __launch_bounds__(128) k_prepass(Grid g, Clock* clk, const double* __restrict__ q1,
-                                                 const double* __restrict__ q2, const double* __restrict__ q3) {
+template <class T>
+__global__ void __launch_bounds__(128) k_prepass(Grid g, Clock* clk, const T* __restrict__ q1, const T* __restrict__ q2,
+                                                 const T* __restrict__ q3) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int i_raw = ((int)blockIdx.x * 4 + warp) * 31 + lane - 1;           // column on the ghost-extended mesh, from -1
     const int i = min(i_raw, g.nx);                                           // (lanes beyond the mesh idle on column nx)
@@ -108,6 +109,20 @@ __global__ void k_fill(double* p, size_t n, double v) {
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = v;
 }
 
+// fp32 contexts: conversion between the standard fp64 state q and the stored planes (rho' = q1 - 1, q2, q3) in fp32.
+__global__ void k_to_f32(const double* __restrict__ q1, const double* __restrict__ q2, const double* __restrict__ q3,
+                         float* __restrict__ r, float* __restrict__ m2, float* __restrict__ m3, size_t n) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        r[i] = (float)(q1[i] - 1.0); m2[i] = (float)q2[i]; m3[i] = (float)q3[i];
+    }
+}
+__global__ void k_from_f32(const float* __restrict__ r, const float* __restrict__ m2, const float* __restrict__ m3,
+                           double* __restrict__ q1, double* __restrict__ q2, double* __restrict__ q3, size_t n) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        q1[i] = 1.0 + (double)r[i]; q2[i] = (double)m2[i]; q3[i] = (double)m3[i];
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 struct fvnl_ctx {
     Grid g;
@@ -118,7 +133,9 @@ struct fvnl_ctx {
     bool own_ws;
     Clock* clk;                 // device clock
     double* src;                // analytic ghost cells of SOURCE sides, two buffers (src_buffer)
-    double* buf[2][3];          // two state buffers (ping-pong); cur = index of the current state
+    int prec;                   // 64 or 32
+    size_t elem;                // bytes of a state value
+    char* buf[2][3];            // two state buffers (ping-pong) of `prec`-bit planes; cur = index of the current state
     int cur;
     double* star[3];            // unfused path only: Q* on the y-extended mesh, allocated on first use
     Clock* host_clk;            // pinned
@@ -181,8 +198,8 @@ static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 static const size_t CLOCK_BYTES = 256;
 
 extern "C" size_t fvnl_workspace_bytes(int nx, int ny, int precision) {
-    if (nx < 4 || ny < 4 || precision != 64) return 0;
-    const size_t plane = align_up((size_t)nx * ny * sizeof(double), 256);
+    if (nx < 4 || ny < 4 || (precision != 64 && precision != 32)) return 0;
+    const size_t plane = align_up((size_t)nx * ny * (precision / 8), 256);
     return CLOCK_BYTES + 6 * plane + align_up(2 * src_stride(nx, ny) * sizeof(double), 256);
 }
 
@@ -197,7 +214,7 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
     if (!out) return FVNL_EARG;
     *out = nullptr;
     if (nx < 4 || ny < 4 || !(dx > 0) || !(dy > 0) || !m || !(m->c0 > 0) || !(m->rho0 > 0) || !(m->beta >= 1) ||
-        !(m->delta >= 0) || precision != 64)
+        !(m->delta >= 0) || (precision != 64 && precision != 32))
         return FVNL_EARG;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { (void)cudaGetLastError(); return FVNL_ECUDA; }
@@ -212,6 +229,8 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
     for (int s = 0; s < 4; ++s) c->g.side[s].kind = BC_EXTRAP;
     c->stream = (cudaStream_t)cuda_stream;
     c->n = (size_t)nx * ny;
+    c->prec = precision;
+    c->elem = precision / 8;
     const size_t need = fvnl_workspace_bytes(nx, ny, precision);
     if (workspace) {
         if (workspace_bytes < need || ((size_t)workspace & 255)) { delete c; return FVNL_EALLOC; }
@@ -220,12 +239,12 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
         if (cudaMalloc(&c->ws, need) != cudaSuccess) { (void)cudaGetLastError(); delete c; return FVNL_EALLOC; }
         c->own_ws = true;
     }
-    const size_t plane = align_up(c->n * sizeof(double), 256);
+    const size_t plane = align_up(c->n * c->elem, 256);
     char* p = (char*)c->ws;
     c->clk = (Clock*)p;
     p += CLOCK_BYTES;
     for (int b = 0; b < 2; ++b)
-        for (int k = 0; k < 3; ++k) { c->buf[b][k] = (double*)p; p += plane; }
+        for (int k = 0; k < 3; ++k) { c->buf[b][k] = p; p += plane; }
     c->src = (double*)p;
     if (cudaMallocHost((void**)&c->host_clk, sizeof(Clock)) != cudaSuccess) {
         (void)cudaGetLastError();
@@ -235,10 +254,11 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
     }
     std::memset(&c->snap, 0, sizeof(Clock));
     bool ok = cudaMemsetAsync(c->clk, 0, CLOCK_BYTES, c->stream) == cudaSuccess;
-    // equilibrium state (1, 0, 0)
+    // equilibrium state: q = (1, 0, 0), stored in fp32 contexts as (rho', q2, q3) = (0, 0, 0)
+    ok = ok && cudaMemsetAsync(c->buf[0][0], 0, plane, c->stream) == cudaSuccess;
     ok = ok && cudaMemsetAsync(c->buf[0][1], 0, plane, c->stream) == cudaSuccess;
     ok = ok && cudaMemsetAsync(c->buf[0][2], 0, plane, c->stream) == cudaSuccess;
-    k_fill<<<592, 256, 0, c->stream>>>(c->buf[0][0], c->n, 1.0);
+    if (c->prec == 64) k_fill<<<592, 256, 0, c->stream>>>((double*)c->buf[0][0], c->n, 1.0);
     ok = ok && cudaGetLastError() == cudaSuccess;
     c->launches = 1;
     c->have_state = true;
@@ -246,7 +266,8 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
     c->kernel = FVNL_KERNEL_DEFAULT;
     c->variant = DEFAULT_VARIANT;
     // per device (function attributes belong to the context of the current device)
-    ok = ok && cudaFuncSetAttribute(k_step_ws, cudaFuncAttributeMaxDynamicSharedMemorySize, ws_smem_bytes()) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(k_step_ws<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, ws_smem_bytes<double>()) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(k_step_ws<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, ws_smem_bytes<float>()) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(k_step_fused<FUSED_BX, FUSED_MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     fused_smem_bytes<FUSED_BX>()) == cudaSuccess;
     if (!ok) { (void)cudaGetLastError(); fvnl_destroy(c); return FVNL_ECUDA; }
@@ -290,6 +311,7 @@ extern "C" int fvnl_set_option(fvnl_ctx* c, int option, int value) {
     c->gvalid = false;
     if (option == FVNL_OPT_KERNEL) {
         if (value != FVNL_KERNEL_DEFAULT && value != FVNL_KERNEL_UNFUSED) return FVNL_EARG;
+        if (value != FVNL_KERNEL_DEFAULT && c->prec != 64) return FVNL_EARG;      // the comparison paths are fp64 only
         c->kernel = value;
         return FVNL_OK;
     }
@@ -299,7 +321,7 @@ extern "C" int fvnl_set_option(fvnl_ctx* c, int option, int value) {
         return FVNL_OK;
     }
     if (option == FVNL_OPT_VARIANT) {
-        if (value < 0 || value >= N_FUSED_VARIANTS) return FVNL_EARG;
+        if (value < 0 || value >= N_FUSED_VARIANTS || (value != 0 && c->prec != 64)) return FVNL_EARG;
         c->variant = value;
         return FVNL_OK;
     }
@@ -310,11 +332,19 @@ extern "C" int fvnl_set_option(fvnl_ctx* c, int option, int value) {
     return FVNL_EARG;
 }
 
-extern "C" int fvnl_set_state(fvnl_ctx* c, const void* q1, const void* q2, const void* q3, int on_device) {
-    if (!c || !q1 || !q2 || !q3) return FVNL_EARG;
+extern "C" int fvnl_set_state(fvnl_ctx* c, const void* q1, const void* q2, const void* q3, int where) {
+    if (!c || !q1 || !q2 || !q3 || where < 0 || where > 3) return FVNL_EARG;
+    const bool on_device = where & FVNL_ON_DEVICE, as_f64 = (where & FVNL_PLANES_F64) && c->prec == 32;
+    if (as_f64 && !on_device) return FVNL_EARG;                   // the conversion runs on the device
     const void* src[3] = {q1, q2, q3};
-    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-    for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(c->buf[c->cur][k], src[k], c->n * sizeof(double), kind, c->stream));
+    if (as_f64) {
+        k_to_f32<<<1184, 256, 0, c->stream>>>((const double*)q1, (const double*)q2, (const double*)q3, (float*)c->buf[c->cur][0],
+                                             (float*)c->buf[c->cur][1], (float*)c->buf[c->cur][2], c->n);
+        c->launches += 1;
+    } else {
+        const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+        for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(c->buf[c->cur][k], src[k], c->n * c->elem, kind, c->stream));
+    }
     // reset sticky flags and the lagged maximum, keep t (and the step counter): on the device, in stream order
     k_clock_reset<<<1, 1, 0, c->stream>>>(c->clk);
     c->launches += 1;
@@ -372,20 +402,29 @@ static int fused_rows(const fvnl_ctx* c, int strips, int slots, int fill = 7) {
 }
 
 // value / mode / more: what the block that finishes last needs to end the step (step_tail).
-static void launch_step(fvnl_ctx* c, double** a, double** b, double value, int mode, int more) {
+static void launch_step(fvnl_ctx* c, char** a, char** b, double value, int mode, int more) {
     const Grid& g = c->g;
     SpanGuard sp(c, FVNL_TIMED_STEP);
     if (c->variant == 0) {
         const int strips = (g.nx + (WS_COLS - 6) - 1) / (WS_COLS - 6);
-        const int rows = fused_rows(c, strips, 148 * WS_BLOCKS_PER_SM, 9);
+        const int per_sm = c->prec == 64 ? WsBudget<double>::blocks_per_sm : WsBudget<float>::blocks_per_sm;
+        const int rows = fused_rows(c, strips, 148 * per_sm, 9);
         const dim3 grd(strips, (g.ny + rows - 1) / rows);
-        k_step_ws<<<grd, 256, ws_smem_bytes(), c->stream>>>(g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows, value, mode, more);
+        if (c->prec == 64)
+            k_step_ws<double><<<grd, 256, ws_smem_bytes<double>(), c->stream>>>(
+                g, c->clk, (const double*)a[0], (const double*)a[1], (const double*)a[2], (double*)b[0], (double*)b[1],
+                (double*)b[2], rows, value, mode, more);
+        else
+            k_step_ws<float><<<grd, 256, ws_smem_bytes<float>(), c->stream>>>(
+                g, c->clk, (const float*)a[0], (const float*)a[1], (const float*)a[2], (float*)b[0], (float*)b[1],
+                (float*)b[2], rows, value, mode, more);
     } else {
         const int strips = (g.nx + (FUSED_BX - 6) - 1) / (FUSED_BX - 6);
         const int rows = fused_rows(c, strips, 148 * FUSED_MINB);
         const dim3 grd(strips, (g.ny + rows - 1) / rows);
         k_step_fused<FUSED_BX, FUSED_MINB><<<grd, FUSED_BX, fused_smem_bytes<FUSED_BX>(), c->stream>>>(
-            g, c->clk, a[0], a[1], a[2], b[0], b[1], b[2], rows, value, mode, more);
+            g, c->clk, (const double*)a[0], (const double*)a[1], (const double*)a[2], (double*)b[0], (double*)b[1],
+            (double*)b[2], rows, value, mode, more);
     }
 }
 
@@ -408,8 +447,8 @@ static void launch_sources(fvnl_ctx* c) {
 // cells of the step that follows (into the other buffer), and the block that finishes last ends the step (clock); only
 // the first step of a call gets its ghost cells from k_sources (the clock may have been set by the host in between).
 static void onepass_step(fvnl_ctx* c, double value, int mode, int more) {
-    double** a = c->buf[c->cur];
-    double** b = c->buf[c->cur ^ 1];
+    char** a = c->buf[c->cur];
+    char** b = c->buf[c->cur ^ 1];
     launch_step(c, a, b, value, mode, more);
     c->cur ^= 1;
     c->launches += 1;
@@ -431,7 +470,9 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
     const int pre = (mode == 1 && c->need_prepass) ? 1 : 0;
     if (pre) {                                                      // O7: M of the current state (k_clock_reset / _set
         const dim3 grd((g.nx + 1 + 123) / 124, (g.ny + PRE_ROWS - 1) / PRE_ROWS);      // left the running maxima at zero)
-        k_prepass<<<grd, 128, 0, st>>>(g, c->clk, c->buf[c->cur][0], c->buf[c->cur][1], c->buf[c->cur][2]);
+        char** q = c->buf[c->cur];
+        if (c->prec == 64) k_prepass<double><<<grd, 128, 0, st>>>(g, c->clk, (const double*)q[0], (const double*)q[1], (const double*)q[2]);
+        else k_prepass<float><<<grd, 128, 0, st>>>(g, c->clk, (const float*)q[0], (const float*)q[1], (const float*)q[2]);
         c->launches += 1;
     }
     k_clock_begin<<<1, 1, 0, st>>>(g, c->clk, value, mode, pre);
@@ -480,8 +521,8 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
             onepass_step(c, value, mode, more);
             continue;
         }
-        double** a = c->buf[c->cur];
-        double** b = c->buf[c->cur ^ 1];
+        double* a[3] = {(double*)c->buf[c->cur][0], (double*)c->buf[c->cur][1], (double*)c->buf[c->cur][2]};
+        double* b[3] = {(double*)c->buf[c->cur ^ 1][0], (double*)c->buf[c->cur ^ 1][1], (double*)c->buf[c->cur ^ 1][2]};
         const dim3 blk(256), grd((g.nx + 255) / 256, g.ny), grdx((g.nx + 255) / 256, g.ny + 4);
         { SpanGuard sp(c, FVNL_TIMED_XSWEEP);
           k_xsweep_unfused<<<grdx, blk, 0, st>>>(g, c->clk, a[0], a[1], a[2], c->star[0], c->star[1], c->star[2]); }
@@ -500,12 +541,21 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
     return c->snap.flags;
 }
 
-extern "C" int fvnl_get_state(fvnl_ctx* c, void* q1, void* q2, void* q3, int on_device) {
-    if (!c || !q1 || !q2 || !q3) return FVNL_EARG;
+extern "C" int fvnl_get_state(fvnl_ctx* c, void* q1, void* q2, void* q3, int where) {
+    if (!c || !q1 || !q2 || !q3 || where < 0 || where > 3) return FVNL_EARG;
     if (!c->have_state) return FVNL_ESTATE;
+    const bool on_device = where & FVNL_ON_DEVICE, as_f64 = (where & FVNL_PLANES_F64) && c->prec == 32;
+    if (as_f64 && !on_device) return FVNL_EARG;
     void* dst[3] = {q1, q2, q3};
+    if (as_f64) {
+        k_from_f32<<<1184, 256, 0, c->stream>>>((const float*)c->buf[c->cur][0], (const float*)c->buf[c->cur][1],
+                                               (const float*)c->buf[c->cur][2], (double*)q1, (double*)q2, (double*)q3, c->n);
+        c->launches += 1;
+        CK(cudaGetLastError());
+        return FVNL_OK;
+    }
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
-    for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(dst[k], c->buf[c->cur][k], c->n * sizeof(double), kind, c->stream));
+    for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(dst[k], c->buf[c->cur][k], c->n * c->elem, kind, c->stream));
     if (!on_device) CK(cudaStreamSynchronize(c->stream));
     return FVNL_OK;
 }

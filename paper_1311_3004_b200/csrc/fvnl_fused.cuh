@@ -69,15 +69,16 @@ __device__ __forceinline__ RowMap map_row(const Grid& g, int r) {
 // Cell (i, r) of the ghost-extended mesh, cm = map_column(g, i): the x rule first, then the y rule (reading A9: a corner
 // is the x-ghost of a y-ghost row); analytic cells of SOURCE sides from the buffer `src` of this step (src_buffer), where
 // a record with q1 <= 0 means "outside the aperture: extrapolate".
+// T = type of the state planes; the cell is returned in full fp64 form (fp32 planes hold rho' = q1 - 1).
+template <class T>
 __device__ __forceinline__ Q3 load_mapped(const Grid& g, const double* __restrict__ src, const ColMap& cm, int i, int r,
-                                          const double* __restrict__ q1, const double* __restrict__ q2,
-                                          const double* __restrict__ q3) {
+                                          const T* __restrict__ q1, const T* __restrict__ q2, const T* __restrict__ q3) {
     const RowMap rm = map_row(g, r);
     const size_t idx = (size_t)rm.row * g.nx + cm.col;
     Q3 c;
-    c.q1 = q1[idx];
-    c.q2 = cm.neg2 ? -q2[idx] : q2[idx];
-    c.q3 = rm.neg3 ? -q3[idx] : q3[idx];
+    c.q1 = Num<T>::perturbation ? 1.0 + (double)q1[idx] : (double)q1[idx];
+    c.q2 = cm.neg2 ? -(double)q2[idx] : (double)q2[idx];
+    c.q3 = rm.neg3 ? -(double)q3[idx] : (double)q3[idx];
     if (cm.xsrc >= 0 && r >= -3 && r <= g.ny + 2) {
         const int l = cm.xsrc == SIDE_XLO ? -1 - i : i - g.nx;
         if (l < 3) {
@@ -144,12 +145,13 @@ __device__ __noinline__ double2 ghost_z(Grid g, int sd, double along, double xc,
 
 // Rolling y-state of one interface (the newest one): its cell on the high side, waves, 1/(r.r), and the limiter
 // inputs it would take from the interface below it (used if that one is its upwind side).
-struct YSet {
-    Cx c;
-    Wv w;
-    double rn1, rn2;
-    double pb1, pb2, pb3;
+template <class T> struct YSetT {
+    CxT<T> c;
+    WvT<T> w;
+    T rn1, rn2;
+    T pb1, pb2, pb3;
 };
+using YSet = YSetT<double>;
 
 // Shared-memory layout: ten arrays of double2, one element per column (+ one pad element on each side so that
 // tid-1 / tid+1 never clamp).  Every access is [p + constant] from ONE per-thread pointer p = base + 16 (tid+1);
@@ -159,9 +161,13 @@ constexpr int SM_ARRAYS = 10;
 template <int BX> __host__ __device__ constexpr int sm_off(int k) { return k * (BX + 2) * 16; }
 
 __device__ __forceinline__ void sts2(char* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
+__device__ __forceinline__ void sts2(char* p, float a, float b) { *reinterpret_cast<float2*>(p) = make_float2(a, b); }
 __device__ __forceinline__ double2 lds2(const char* p) { return *reinterpret_cast<const double2*>(p); }
 __device__ __forceinline__ void sts1(char* p, double a) { *reinterpret_cast<double*>(p) = a; }
+__device__ __forceinline__ void sts1(char* p, float a) { *reinterpret_cast<float*>(p) = a; }
 __device__ __forceinline__ double lds1(const char* p) { return *reinterpret_cast<const double*>(p); }
+template <class T> __device__ __forceinline__ typename Num<T>::T2 ldp(const char* p) { return *reinterpret_cast<const typename Num<T>::T2*>(p); }
+template <class T> __device__ __forceinline__ T ld1(const char* p) { return *reinterpret_cast<const T*>(p); }
 
 // Rows of Q^n are prefetched two ticks ahead with cp.async (LDGSTS) into a four-slot ring of shared memory, each
 // thread copying and later reading only its own three values -- no barrier needed, no registers held by loads in
@@ -170,19 +176,26 @@ __device__ __forceinline__ void cp_async8(char* smem_dst, const double* gsrc) {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
 }
+__device__ __forceinline__ void cp_async_elem(char* smem_dst, const double* gsrc) { cp_async8(smem_dst, gsrc); }
+__device__ __forceinline__ void cp_async_elem(char* smem_dst, const float* gsrc) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 template <int BX> __host__ __device__ constexpr int pre_slot_bytes() { return 3 * BX * 8; }
 
 // Block-invariant quantities of a step.
-struct StepK {
-    double t, lamx, lamy, kapx, kapy, k2;    // k2 = -2 (kapx + kapy)
-    double b2, omb2;                         // 2 (beta - 1), 1 - b2
+template <class T> struct StepKT {
+    double t;
+    T lamx, lamy, kapx, kapy, k2;            // k2 = -2 (kapx + kapy)
+    T b2, omb2;                              // 2 (beta - 1), 1 - b2
     int j0, j1;                              // rows of output of this chunk: [j0, j1)
     int ylo, ycnt;                           // y-interface ry-1/2 is one the scheme solves iff (unsigned)(ry-ylo) <= ycnt
     bool px, py, any_src, any_refl;
     const double* src;                       // analytic ghost cells of this step (k_step_ws), see src_buffer
 };
+using StepK = StepKT<double>;
 
 // Per-thread constants and running reductions.
 struct ThreadK {

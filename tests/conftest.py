@@ -30,3 +30,17 @@ def read_golden_kv(name):
 @pytest.fixture(scope="session")
 def golden_dir():
     return GOLDEN
+
+
+_ORACLE_RUNS = {}
+
+
+def oracle_run_cached(key, w, steps=None):
+    """The oracle's result for a (full-size) workload, computed once per pytest session and shared by the fp64 and fp32
+    parity tests: (state after `steps`, info, flags)."""
+    if key not in _ORACLE_RUNS:
+        from helpers import oracle_from_workload
+        o = oracle_from_workload(w, threads=0)
+        flags = o.step(w.steps if steps is None else steps, w.value, w.mode)
+        _ORACLE_RUNS[key] = (o.get_state(), o.info(), flags)
+    return _ORACLE_RUNS[key]

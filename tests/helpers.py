@@ -13,10 +13,10 @@ def oracle_from_workload(w, threads=0, state=None):
     return o
 
 
-def solver_from_workload(w, state=None, device="cuda"):
+def solver_from_workload(w, state=None, device="cuda", precision=64):
     import torch
     from paper_1311_3004_b200 import Solver
-    s = Solver(w.nx, w.ny, w.dx, w.dy, **w.medium, device=device)
+    s = Solver(w.nx, w.ny, w.dx, w.dy, **w.medium, device=device, precision=precision)
     for side, (kind, src) in enumerate(w.bc):
         s.set_bc(side, kind, src)
     if state is None:

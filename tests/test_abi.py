@@ -40,7 +40,8 @@ def test_host_side_checks_without_a_device():
     import torch
     import paper_1311_3004_b200 as P
     assert P.fvnl_workspace_bytes(3, 8) == 0
-    assert P.fvnl_workspace_bytes(8, 8, 32) == 0
+    assert P.fvnl_workspace_bytes(8, 8, 16) == 0
+    assert 0 < P.fvnl_workspace_bytes(1024, 1024, 32) < P.fvnl_workspace_bytes(1024, 1024, 64) * 0.52
     n = P.fvnl_workspace_bytes(1024, 1024)
     # clock + two states + the analytic ghost cells of the edges (9 doubles per edge cell, two buffers), nothing else
     assert n >= 6 * 1024 * 1024 * 8 and n < 6 * 1024 * 1024 * 8 + 4096 + 2 * (9 * 8 * (4 * 1024 + 12) + 256)
