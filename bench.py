@@ -147,11 +147,15 @@ def measured_peaks():
 
 # ---------------------------------------------------------------------------------------------------------------
 # CPU legs: the oracle as it stands (oracle/, never tuned), on the host cores.  Only these two functions touch it.
-def _oracle_sample(w_full, n_sample):
-    """A bounded sample of the same workload: the workload's own generator at n_sample^2 cells."""
+ORACLE_SAMPLE_N = 2048      # one sample size for the cpu_baseline leg and the reference arm (the oracle's rate depends on it)
+
+
+def _oracle_sample(w_full, n_sample=ORACLE_SAMPLE_N):
+    """A bounded sample of the same workload: the workload's own generator (and seed) at n_sample^2 cells."""
     import workloads as W
     if w_full.name.startswith(("C5", "C3")):
-        return W.c3_random(n=n_sample, steps=1, nu_w=w_full.value, seed=1311300499, name=f"{w_full.name}@{n_sample}^2")
+        return W.c3_random(n=min(n_sample, w_full.nx), steps=1, nu_w=w_full.value, seed=w_full.extra["seed"],
+                           name=f"{w_full.name}@{min(n_sample, w_full.nx)}^2")
     if w_full.name == "C2":
         return W.c2_pulse(n=n_sample, steps=1)
     if w_full.name == "C4":
@@ -175,8 +179,7 @@ def cpu_baseline(w_full, budget_s=12.0):
     o.step(1, ws.value, ws.mode)                                   # includes the pre-pass; warm-up
     t0 = time.perf_counter(); o.step(1, ws.value, ws.mode); t1 = time.perf_counter()
     rate = ws.cells / (t1 - t0)
-    n = 2048
-    ws = _oracle_sample(w_full, n)
+    ws = _oracle_sample(w_full)
     steps = int(max(1, min(200, round(budget_s * rate / ws.cells))))
     o = oracle_context(ws)
     o.step(1, ws.value, ws.mode)
@@ -192,8 +195,7 @@ def run_reference(args):
     if rank != 0:
         return
     w_full = make_workload(args.workload)
-    n = 1024
-    ws = _oracle_sample(w_full, n)
+    ws = _oracle_sample(w_full)
     o = oracle_context(ws)
     o.step(max(1, args.warmup), ws.value, ws.mode)
     t0 = time.perf_counter(); o.step(args.steps, ws.value, ws.mode); t1 = time.perf_counter()

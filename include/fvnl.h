@@ -66,9 +66,11 @@ enum { FVNL_SIDE_XLO = 0, FVNL_SIDE_XHI = 1, FVNL_SIDE_YLO = 2, FVNL_SIDE_YHI = 
  *     (focus_m <= 0 or infinite: plane wave, tau has no d term, normal momentum = g, along-edge momentum = 0).
  *   Both ghost layers of the edge take the same values (they sample (43) at the edge, A14).  Cells with
  *   |d| > half_aperture_m (> 0) behave as FVNL_BC_EXTRAP; half_aperture_m <= 0: the whole edge.
- *     TANH  : q1 = 1 - amp*tanh(steep*(x - c0*(t + t0_s))), q2 = q1 - 1, q3 = 0        (41)
- *   with x = the x coordinate of the ghost cell's OWN centre measured from the x-lo edge (negative in the x-lo
- *   ghosts): (41) is a field, the same on whichever side it is attached to.  steep [1/m].
+ *     TANH  : q1 = 1 - amp*tanh(steep*(xi - c0*(t + t0_s))), (q2, q3) = (q1 - 1)*(cos theta, sin theta)   (41)
+ *   with xi = x*cos(theta) + y*sin(theta), (x, y) = the ghost cell's OWN centre measured from the x-lo / y-lo edge
+ *   (negative in the low ghosts; x in the frame that fvnl_shift moves): (41) is a field, the same on whichever side it is
+ *   attached to.  theta = theta_T, the propagation angle from the x axis (0: q2 = q1 - 1, q3 = 0 as printed).
+ *   steep [1/m].
  *   Sources are evaluated at t_n, the time at the start of the step. */
 enum { FVNL_SRC_SINE = 0, FVNL_SRC_PACKET = 1, FVNL_SRC_TANH = 2 };
 typedef struct {
@@ -80,6 +82,7 @@ typedef struct {
     double half_aperture_m; /* a of PAPER.md:405; <= 0: whole edge                                     */
     double t0_s;
     double steep;           /* TANH only                                                               */
+    double theta;           /* TANH only: propagation angle theta_T [rad]                              */
 } fvnl_source;
 
 /* Precision of a context.  64: the paper's, state planes of double holding q.  32: the single-precision
@@ -121,6 +124,16 @@ enum { FVNL_ON_HOST = 0, FVNL_ON_DEVICE = 1, FVNL_PLANES_F64 = 2 };
  * be reused when it returns. */
 int fvnl_set_state(fvnl_ctx* ctx, const void* q1_dev_or_host, const void* q2_dev_or_host,
                    const void* q3_dev_or_host, int where);
+
+/* Moving domain, the second stage of PAPER.md:281-287 ("the domain moves with the propagation wave"): move the domain by
+ * `cells` >= 0 cells in +x.  The state is re-indexed, Q_new(i, j) = Q_old(i + cells, j); the columns that enter on the right
+ * are the x-hi ghost cells of the old state by the x-hi rule at the current time (EXTRAP: copies of the last column;
+ * SOURCE: the analytic cell at its own centre, inside the aperture), and the frame in which TANH sources are written
+ * moves along.  t and the lagged M are untouched.  Asynchronous (one kernel on the stream).  The caller decides when to
+ * move (e.g. one cell each time c0*t has advanced by dx) and which rule the x-lo edge follows in this stage (the paper:
+ * zero-order extrapolation).
+ * Errors: FVNL_EARG (cells < 0 or >= nx; x edges PERIODIC, x-hi REFLECT), FVNL_ESTATE. */
+int fvnl_shift(fvnl_ctx* ctx, int cells);
 
 /* Set the clock: simulation time t [s] and the lagged maximum M [1/m] of the previous step.
  * last_M <= 0: M unknown -- the next CFL-mode step recomputes it by the pre-pass on the state as it is then, unless a

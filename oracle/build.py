@@ -15,9 +15,15 @@ LIB = os.path.join(HERE, "libfvnl_oracle.so")
 def build(force: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
         return LIB
+    tmp = f"{LIB}.{os.getpid()}.tmp"                  # appear atomically: a running process keeps its mapped copy
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
-           "-shared", "-fPIC", "-o", LIB, SRC]
-    subprocess.run(cmd, check=True)
+           "-shared", "-fPIC", "-o", tmp, SRC]
+    try:
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, LIB)
+    finally:
+        if os.path.exists(tmp):
+            os.remove(tmp)
     return LIB
 
 

@@ -52,6 +52,7 @@ enum { SIDE_XLO = 0, SIDE_XHI = 1, SIDE_YLO = 2, SIDE_YHI = 3 };
 struct Source {
     int shape;
     double amp, freq_hz, focus_m, centre_m, half_aperture_m, t0_s, steep;
+    double theta;     // TANH only: propagation angle theta_T from the x_1 axis
 };
 
 struct Cell { double q[3]; };
@@ -188,6 +189,8 @@ struct Oracle {
     Source src[4];
     std::vector<double> q[3];
     double t, M_prev, last_dt, last_cfl;
+    double x_origin;  // x of the x-lo edge in the frame in which the travelling profile (41) is written; moves with the
+                      // domain in the second stage
     long steps;
     int flags;
     int nthreads;
@@ -199,15 +202,20 @@ inline Cell load(const std::vector<double>* q, size_t idx) {
 
 // Boundary source cell.  (41) PAPER.md:330 ; (43a-d) PAPER.md:409-418 ; readings A11, A13, A14, A16.
 // side: which edge the ghost cell belongs to.  along_m: coordinate of the cell centre along that edge, measured
-// from the low corner.  xc_m: x of the ghost cell's own centre measured from the x-lo edge (TANH only).
+// from the low corner.  xc_m, yc_m: x and y of the ghost cell's own centre measured from the x-lo / y-lo edge (TANH only).
 // Returns false if the cell lies outside the aperture (then it behaves as EXTRAP).
-bool source_cell(const Oracle& o, int side, double along_m, double xc_m, double t, Cell* out) {
+bool source_cell(const Oracle& o, int side, double along_m, double xc_m, double yc_m, double t, Cell* out) {
     const Source& s = o.src[side];
     const double PI = 3.14159265358979323846;
     if (s.shape == SRC_TANH) {
-        // q1 = 1 - (delta~/beta) tanh(x - t) in the paper's units; "steep" carries the 10%-90% width (A11).
-        const double q1 = 1.0 - s.amp * std::tanh(s.steep * (xc_m - o.c0 * (t + s.t0_s)));
-        out->q[0] = q1; out->q[1] = q1 - 1.0; out->q[2] = 0.0;
+        // q1 = 1 - (delta~/beta) tanh(x - t), q2 = q1 - 1, q3 = 0 in the paper's units (41); "steep" carries the 10%-90%
+        // width (A11).  Propagation at an angle theta_T from the x_1 axis: "to use them with a different value of theta_T,
+        // we have applied a standard rotation change of variables": x -> the coordinate along the
+        // propagation direction, x cos(theta) + y sin(theta); the velocity (q2, q3) -> its rotation by theta.
+        const double ct = std::cos(s.theta), st = std::sin(s.theta);
+        const double xi = (o.x_origin + xc_m) * ct + yc_m * st;
+        const double q1 = 1.0 - s.amp * std::tanh(s.steep * (xi - o.c0 * (t + s.t0_s)));
+        out->q[0] = q1; out->q[1] = (q1 - 1.0) * ct; out->q[2] = (q1 - 1.0) * st + 0.0;
         return true;
     }
     const double d = along_m - s.centre_m;                       // x_2 of (43), from the aperture centre
@@ -266,12 +274,12 @@ void ghosts(const Oracle& o, int axis, int fixed, const Cell* line, int n, int g
                 c = e ? line[n - 1] : line[0];                    // zero-order extrapolation
                 if (kind == BC_SOURCE) {
                     const double along = (fixed + 0.5) * h_along;
-                    // x of this ghost cell's own centre from the x-lo edge (TANH)
-                    double xc;
-                    if (axis == 0) xc = e ? (o.nx + k + 0.5) * o.dx : -(k + 0.5) * o.dx;
-                    else           xc = (fixed + 0.5) * o.dx;
+                    // x, y of this ghost cell's own centre from the x-lo / y-lo edge (TANH)
+                    double xc, yc;
+                    if (axis == 0) { xc = e ? (o.nx + k + 0.5) * o.dx : -(k + 0.5) * o.dx; yc = (fixed + 0.5) * o.dy; }
+                    else           { xc = (fixed + 0.5) * o.dx; yc = e ? (o.ny + k + 0.5) * o.dy : -(k + 0.5) * o.dy; }
                     Cell sc;
-                    if (source_cell(o, side, along, xc, t, &sc)) c = sc;
+                    if (source_cell(o, side, along, xc, yc, t, &sc)) c = sc;
                 }
             }
             G[k] = c;
@@ -443,7 +451,7 @@ void source_step(Oracle& o, double dt) {
 extern "C" {
 
 struct orc_medium { double c0, rho0, beta, delta; };
-struct orc_source { int shape; double amp, freq_hz, focus_m, centre_m, half_aperture_m, t0_s, steep; };
+struct orc_source { int shape; double amp, freq_hz, focus_m, centre_m, half_aperture_m, t0_s, steep, theta; };
 
 void* orc_create(int nx, int ny, double dx, double dy, const orc_medium* m) {
     if (nx < 4 || ny < 4 || !(dx > 0) || !(dy > 0) || !m || !(m->c0 > 0) || !(m->rho0 > 0) || !(m->beta >= 1) || !(m->delta >= 0))
@@ -454,6 +462,7 @@ void* orc_create(int nx, int ny, double dx, double dy, const orc_medium* m) {
     for (int s = 0; s < 4; ++s) { o->bc[s] = BC_EXTRAP; std::memset(&o->src[s], 0, sizeof(Source)); }
     for (int k = 0; k < 3; ++k) o->q[k].assign((size_t)nx * ny, k == 0 ? 1.0 : 0.0);
     o->t = 0.0; o->M_prev = 0.0; o->last_dt = 0.0; o->last_cfl = 0.0; o->steps = 0; o->flags = 0;
+    o->x_origin = 0.0;
     o->nthreads = 1;
     return o;
 }
@@ -478,7 +487,7 @@ int orc_set_bc(void* h, int side, int kind, const orc_source* s) {
         if (!s) return ORC_EARG;
         Source& d = o->src[side];
         d.shape = s->shape; d.amp = s->amp; d.freq_hz = s->freq_hz; d.focus_m = s->focus_m; d.centre_m = s->centre_m;
-        d.half_aperture_m = s->half_aperture_m; d.t0_s = s->t0_s; d.steep = s->steep;
+        d.half_aperture_m = s->half_aperture_m; d.t0_s = s->t0_s; d.steep = s->steep; d.theta = s->theta;
     }
     o->bc[side] = kind;
     return ORC_OK;
@@ -568,11 +577,34 @@ int orc_sweep_line(int n, const double* cells, double lam, double beta, double* 
     return flag;
 }
 
+// Second stage of PAPER.md:287: "the domain moves with the propagation wave".  Move the domain by k cells in +x: the
+// state is re-indexed, Q_new(i, j) = Q_old(i + k, j), the k columns that enter on the right are the x-hi ghost cells of the
+// old state by the x-hi rule at the current time (zero-order extrapolation, or the analytic profile (41) at their own
+// centres), and the frame of (41) moves along (x_origin).  The clock (t, lagged M) is untouched.
+int orc_shift(void* h, int k) {
+    Oracle* o = static_cast<Oracle*>(h);
+    if (k < 0 || k >= o->nx) return ORC_EARG;
+    if (o->bc[SIDE_XLO] == BC_PERIODIC || o->bc[SIDE_XHI] == BC_PERIODIC || o->bc[SIDE_XHI] == BC_REFLECT) return ORC_EARG;
+    if (k == 0) return ORC_OK;
+    const int nx = o->nx, ny = o->ny;
+    std::vector<Cell> row(nx), lo(k), hi(k);
+    for (int j = 0; j < ny; ++j) {
+        for (int i = 0; i < nx; ++i) row[i] = load(o->q, (size_t)j * nx + i);
+        ghosts(*o, 0, j, row.data(), nx, k, o->t, lo.data(), hi.data());
+        for (int i = 0; i < nx; ++i) {
+            const Cell& c = (i + k < nx) ? row[i + k] : hi[i + k - nx];
+            for (int m = 0; m < 3; ++m) o->q[m][(size_t)j * nx + i] = c.q[m];
+        }
+    }
+    o->x_origin += k * o->dx;
+    return ORC_OK;
+}
+
 // boundary source cell as the ghost rule evaluates it (for tests of (41)/(43))
-int orc_source_cell(void* h, int side, double along_m, double xc_m, double t, double out[3]) {
+int orc_source_cell(void* h, int side, double along_m, double xc_m, double yc_m, double t, double out[3]) {
     Oracle* o = static_cast<Oracle*>(h);
     Cell c;
-    const bool in = source_cell(*o, side, along_m, xc_m, t, &c);
+    const bool in = source_cell(*o, side, along_m, xc_m, yc_m, t, &c);
     if (in) { out[0] = c.q[0]; out[1] = c.q[1]; out[2] = c.q[2]; }
     return in ? 1 : 0;
 }

@@ -21,7 +21,7 @@ class _Medium(C.Structure):
 class OrcSource(C.Structure):
     _fields_ = [("shape", C.c_int), ("amp", C.c_double), ("freq_hz", C.c_double), ("focus_m", C.c_double),
                 ("centre_m", C.c_double), ("half_aperture_m", C.c_double), ("t0_s", C.c_double),
-                ("steep", C.c_double)]
+                ("steep", C.c_double), ("theta", C.c_double)]
 
 
 _lib = None
@@ -48,7 +48,8 @@ def lib():
         L.orc_mc_phi.restype = C.c_double
         L.orc_mc_phi.argtypes = [C.c_double]
         L.orc_sweep_line.argtypes = [C.c_int, _dp, C.c_double, C.c_double, _dp, _dp]
-        L.orc_source_cell.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double, _dp]
+        L.orc_source_cell.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, _dp]
+        L.orc_shift.argtypes = [C.c_void_p, C.c_int]
         L.orc_prepass.restype = C.c_double
         L.orc_prepass.argtypes = [C.c_void_p]
         _lib = L
@@ -116,10 +117,16 @@ class Oracle:
     def prepass(self):
         return lib().orc_prepass(self._h)
 
-    def source_cell(self, side, along_m, xc_m, t):
+    def source_cell(self, side, along_m, xc_m, t, yc_m=0.0):
         out = np.zeros(3)
-        inside = lib().orc_source_cell(self._h, side, along_m, xc_m, t, _p(out))
+        inside = lib().orc_source_cell(self._h, side, along_m, xc_m, yc_m, t, _p(out))
         return bool(inside), out
+
+    def shift(self, cells):
+        """Move the domain by `cells` cells in +x (second stage of PAPER.md:287)."""
+        rc = lib().orc_shift(self._h, int(cells))
+        if rc:
+            raise ValueError(f"orc_shift -> {rc}")
 
 
 def flux(q, beta, direction):

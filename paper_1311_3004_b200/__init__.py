@@ -38,7 +38,7 @@ class fvnl_medium(C.Structure):
 class fvnl_source(C.Structure):
     _fields_ = [("shape", C.c_int), ("amp", C.c_double), ("freq_hz", C.c_double), ("focus_m", C.c_double),
                 ("centre_m", C.c_double), ("half_aperture_m", C.c_double), ("t0_s", C.c_double),
-                ("steep", C.c_double)]
+                ("steep", C.c_double), ("theta", C.c_double)]
 
 
 class FvnlError(RuntimeError):
@@ -66,6 +66,7 @@ def lib():
         L.fvnl_set_option.argtypes = [_vp, C.c_int, C.c_int]
         L.fvnl_set_state.argtypes = [_vp, _vp, _vp, _vp, C.c_int]
         L.fvnl_set_clock.argtypes = [_vp, C.c_double, C.c_double]
+        L.fvnl_shift.argtypes = [_vp, C.c_int]
         L.fvnl_step.argtypes = [_vp, C.c_long, C.c_double, C.c_int]
         L.fvnl_get_state.argtypes = [_vp, _vp, _vp, _vp, C.c_int]
         L.fvnl_get_info.argtypes = [_vp] + [C.POINTER(C.c_double)] * 4 + [C.POINTER(C.c_long)]
@@ -105,6 +106,10 @@ def fvnl_set_option(h, option, value):
 
 def fvnl_set_state(h, p1, p2, p3, where):
     return lib().fvnl_set_state(h, _vp(p1), _vp(p2), _vp(p3), int(where))
+
+
+def fvnl_shift(h, cells):
+    return lib().fvnl_shift(h, int(cells))
 
 
 def fvnl_set_clock(h, t_s, last_M):
@@ -223,6 +228,10 @@ class Solver:
             self._check("fvnl_set_state", fvnl_set_state(self._h, q[0].data_ptr(), q[1].data_ptr(), q[2].data_ptr(), where))
             if where & PLANES_F64:
                 self._stream.synchronize()                             # the temporaries above are read asynchronously
+
+    def shift(self, cells):
+        """Move the domain by `cells` cells in +x (second stage of PAPER.md:287)."""
+        self._check("fvnl_shift", fvnl_shift(self._h, cells))
 
     def set_clock(self, t, last_M=0.0):
         self._check("fvnl_set_clock", fvnl_set_clock(self._h, t, last_M))

@@ -123,6 +123,27 @@ __global__ void k_from_f32(const float* __restrict__ r, const float* __restrict_
     }
 }
 
+// fvnl_shift: the domain moves k cells in +x (second stage of PAPER.md:287).  Q_new(i, j) = Q_old(i + k, j); the k columns
+// that enter on the right are the x-hi ghost cells of the old state by the x-hi rule at the current time: zero-order
+// extrapolation, or the analytic cell at its own centre (inside the aperture).  One thread per cell.
+template <class T>
+__global__ void __launch_bounds__(256) k_shift(Grid g, const Clock* clk, int k, const T* __restrict__ a1, const T* __restrict__ a2,
+                                               const T* __restrict__ a3, T* __restrict__ o1, T* __restrict__ o2,
+                                               T* __restrict__ o3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= g.nx) return;
+    const size_t o = (size_t)j * g.nx + i;
+    const int io = i + k;
+    if (io < g.nx) { o1[o] = a1[o + k]; o2[o] = a2[o + k]; o3[o] = a3[o + k]; return; }
+    const size_t e = (size_t)j * g.nx + g.nx - 1;
+    T c1 = a1[e], c2 = a2[e], c3 = a3[e];
+    Q3 s;
+    if (g.side[SIDE_XHI].kind == BC_SOURCE && source_at(g, SIDE_XHI, io, j, clk->t, s)) {
+        c1 = dens_var<T>(s.q1); c2 = T(s.q2); c3 = T(s.q3);
+    }
+    o1[o] = c1; o2[o] = c2; o3[o] = c3;
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 struct fvnl_ctx {
     Grid g;
@@ -299,7 +320,7 @@ extern "C" int fvnl_set_bc(fvnl_ctx* c, int side, int kind, const fvnl_source* s
         if (!s || s->shape < 0 || s->shape > 2) return FVNL_EARG;
         if (s->shape != SRC_TANH && !(s->freq_hz > 0)) return FVNL_EARG;
         d.shape = s->shape; d.amp = s->amp; d.freq_hz = s->freq_hz; d.focus_m = s->focus_m; d.centre_m = s->centre_m;
-        d.half_aperture_m = s->half_aperture_m; d.t0_s = s->t0_s; d.steep = s->steep;
+        d.half_aperture_m = s->half_aperture_m; d.t0_s = s->t0_s; d.steep = s->steep; d.theta = s->theta;
     }
     c->g.side[side] = d;
     c->gvalid = false;
@@ -354,6 +375,30 @@ extern "C" int fvnl_set_state(fvnl_ctx* c, const void* q1, const void* q2, const
     CK(cudaGetLastError());
     c->have_state = true;
     c->need_prepass = true;
+    return FVNL_OK;
+}
+
+extern "C" int fvnl_shift(fvnl_ctx* c, int cells) {
+    if (!c || cells < 0 || cells >= c->g.nx) return FVNL_EARG;
+    const Grid& g = c->g;
+    if (g.side[SIDE_XLO].kind == BC_PERIODIC || g.side[SIDE_XHI].kind == BC_PERIODIC || g.side[SIDE_XHI].kind == BC_REFLECT)
+        return FVNL_EARG;
+    if (!c->have_state) return FVNL_ESTATE;
+    if (cells == 0) return FVNL_OK;
+    char** a = c->buf[c->cur];
+    char** b = c->buf[c->cur ^ 1];
+    const dim3 grd((g.nx + 255) / 256, g.ny);
+    if (c->prec == 64)
+        k_shift<double><<<grd, 256, 0, c->stream>>>(g, c->clk, cells, (const double*)a[0], (const double*)a[1], (const double*)a[2],
+                                                    (double*)b[0], (double*)b[1], (double*)b[2]);
+    else
+        k_shift<float><<<grd, 256, 0, c->stream>>>(g, c->clk, cells, (const float*)a[0], (const float*)a[1], (const float*)a[2],
+                                                   (float*)b[0], (float*)b[1], (float*)b[2]);
+    CK(cudaGetLastError());
+    c->launches += 1;
+    c->cur ^= 1;
+    c->g.x0 += cells * g.dx;
+    c->gvalid = false;                                             // (a captured graph holds the old frame)
     return FVNL_OK;
 }
 

@@ -14,13 +14,14 @@ enum { SIDE_XLO = 0, SIDE_XHI = 1, SIDE_YLO = 2, SIDE_YHI = 3 };
 
 struct Side {
     int kind, shape;
-    double amp, freq_hz, focus_m, centre_m, half_aperture_m, t0_s, steep;
+    double amp, freq_hz, focus_m, centre_m, half_aperture_m, t0_s, steep, theta;
 };
 
 // Everything a kernel needs to know about the problem; passed by value (kernel parameter space).
 struct Grid {
     int nx, ny;
     double dx, dy, c0, beta, delta;
+    double x0;                  // x of the x-lo edge in the frame of the travelling profile (41); moves with fvnl_shift
     Side side[4];
     double* src;                // analytic ghost cells of SOURCE sides: two buffers (below), null without a SOURCE side
 };
@@ -95,10 +96,13 @@ struct Q3 {
 // Analytic boundary cell: the value an edge of kind SOURCE prescribes for one of its ghost cells at time t.
 //   side   the edge the ghost cell belongs to;
 //   along  coordinate of the cell's centre along that edge, from the low corner [m];
-//   xc     x of the cell's own centre, from the x-lo edge [m] (used by the travelling profile (41) only).
+//   xc, yc the cell's own centre [m]: x in the frame of the profile (41) (Grid::x0 + distance from the x-lo edge), y from the
+//          y-lo edge (used by the travelling profile only).
 // Returns false for a cell outside the aperture: it then follows the extrapolation rule.
 //
-// (41), PAPER.md:330 (reading A11): the travelling profile q1 = 1 - K tanh(k (x - c0 t')), q2 = q1 - 1, q3 = 0.
+// (41), PAPER.md:330 (reading A11): the travelling profile rho' = -K tanh(k (xi - c0 t')) moving along the unit vector
+// e = (cos theta_T, sin theta_T), xi = (x, y).e ("a standard rotation change of variables"), with the
+// velocity along e: (q2, q3) = rho' e  (theta_T = 0: q2 = q1 - 1, q3 = 0 as printed).
 //
 // (43a-d), written from the geometry the paper describes rather than from its component formulas:
 // the transducer is a circular arc centred on the focus; the focus lies at distance F from the edge on the inward normal
@@ -108,11 +112,16 @@ struct Q3 {
 // the centre by the extra path, in the paraxial form the paper gives:  phase = f t' + x2^2 / (2 F lambda)  [periods].
 // g = A sin(2 pi phase) (piston, switched on at phase 0) or the same carrier under the packet envelope exp(-(phase/4)^10)
 // (reading A13).  F <= 0 or infinite: plane wave, direction n, no phase lead.
-__device__ __noinline__ bool source_cell(const Side& s, int side, double c0, double along, double xc, double t, Q3& out) {
+__device__ __noinline__ bool source_cell(const Side& s, int side, double c0, double along, double xc, double yc, double t,
+                                         Q3& out) {
     const double tp = t + s.t0_s;
     if (s.shape == SRC_TANH) {
-        const double rho1 = -s.amp * tanh(s.steep * fma(-c0, tp, xc));                // q1 - 1
-        out.q1 = 1.0 + rho1; out.q2 = out.q1 - 1.0; out.q3 = 0.0;
+        double e_y, e_x;
+        sincos(s.theta, &e_y, &e_x);
+        const double xi = fma(xc, e_x, yc * e_y);
+        out.q1 = 1.0 - s.amp * tanh(s.steep * fma(-c0, tp, xi));
+        const double rho1 = out.q1 - 1.0;                                             // of the ROUNDED q1, as (41) has it
+        out.q2 = rho1 * e_x; out.q3 = rho1 * e_y + 0.0;
         return true;
     }
     const double x2 = along - s.centre_m;
@@ -140,6 +149,12 @@ __device__ __noinline__ bool source_cell(const Side& s, int side, double c0, dou
     return true;
 }
 
+// The analytic cell of SOURCE side sd at position (column i, row r) of the ghost-extended mesh.
+__device__ __forceinline__ bool source_at(const Grid& g, int sd, int i, int r, double t, Q3& out) {
+    const double x = (i + 0.5) * g.dx, y = (r + 0.5) * g.dy;
+    return source_cell(g.side[sd], sd, g.c0, sd < 2 ? y : x, g.x0 + x, y, t, out);
+}
+
 // Record n of Grid::src (layout above): the analytic cell of one ghost position at time t; q1 = -1 marks "outside the
 // aperture".  n < src_off(nx, ny, 4) / 3.
 __device__ __forceinline__ void source_record(const Grid& g, double t, size_t n, double* __restrict__ out) {
@@ -152,13 +167,8 @@ __device__ __forceinline__ void source_record(const Grid& g, double t, size_t n,
             const int layer = (int)(m / per), pos = (int)(m % per);
             Q3 c;
             bool in;
-            if (sd < 2) {
-                const int r = pos - 3, i = sd == SIDE_XLO ? -1 - layer : g.nx + layer;
-                in = source_cell(g.side[sd], sd, g.c0, (r + 0.5) * g.dy, (i + 0.5) * g.dx, t, c);
-            } else {
-                const double x = (pos + 0.5) * g.dx;
-                in = source_cell(g.side[sd], sd, g.c0, x, x, t, c);
-            }
+            if (sd < 2) in = source_at(g, sd, sd == SIDE_XLO ? -1 - layer : g.nx + layer, pos - 3, t, c);
+            else in = source_at(g, sd, pos, sd == SIDE_YLO ? -1 - layer : g.ny + layer, t, c);
             double* o = out + 3 * n;
             o[0] = in ? c.q1 : -1.0; o[1] = in ? c.q2 : 0.0; o[2] = in ? c.q3 : 0.0;
             return;
@@ -190,7 +200,7 @@ __device__ __forceinline__ Q3 load_ext(const Grid& g, const double* __restrict__
         } else {
             if (kind == BC_SOURCE) {
                 Q3 c;
-                if (source_cell(g.side[sd], sd, g.c0, (r + 0.5) * g.dy, (i + 0.5) * g.dx, t, c)) return c;
+                if (source_at(g, sd, i, r, t, c)) return c;
             }
             i = clampi(i, g.nx);
         }
@@ -206,7 +216,7 @@ __device__ __forceinline__ Q3 load_ext(const Grid& g, const double* __restrict__
         } else {
             if (kind == BC_SOURCE) {
                 Q3 c;
-                if (source_cell(g.side[sd], sd, g.c0, (i + 0.5) * g.dx, (i + 0.5) * g.dx, t, c)) {
+                if (source_at(g, sd, i, r, t, c)) {
                     if (neg2) c.q2 = -c.q2;
                     return c;
                 }
@@ -226,15 +236,15 @@ __device__ __forceinline__ Q3 load_ext(const Grid& g, const double* __restrict__
 
 // One-deep ghost of an intermediate state for the source step (26) (reading A9): the rule of `sd` applied to the
 // interior value `inner` (the cell next to the edge, or the wrapped one for PERIODIC -- the caller passes it).
-// `along`, `xc`: as for source_cell.
-__device__ __forceinline__ Q3 ghost_of(const Grid& g, int sd, const Q3& inner, double along, double xc, double t) {
+// (i, r): the ghost cell's position on the ghost-extended mesh.
+__device__ __forceinline__ Q3 ghost_of(const Grid& g, int sd, const Q3& inner, int i, int r, double t) {
     const int kind = g.side[sd].kind;
     Q3 c = inner;
     if (kind == BC_REFLECT) {
         if (sd < 2) c.q2 = -c.q2; else c.q3 = -c.q3;
     } else if (kind == BC_SOURCE) {
         Q3 s;
-        if (source_cell(g.side[sd], sd, g.c0, along, xc, t, s)) c = s;
+        if (source_at(g, sd, i, r, t, s)) c = s;
     }
     return c;
 }

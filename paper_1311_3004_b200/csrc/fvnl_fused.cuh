@@ -118,24 +118,21 @@ __device__ __forceinline__ bool step_tail(const Grid& g, Clock* clk, double valu
 __device__ __noinline__ double3 apply_sources(Grid g, int xsrc, int ysrc, int col, bool neg2, int i, int r, double t,
                                               double c1, double c2, double c3) {
     Q3 s;
-    if (xsrc >= 0 && source_cell(g.side[xsrc], xsrc, g.c0, (r + 0.5) * g.dy, (i + 0.5) * g.dx, t, s))
-        return make_double3(s.q1, s.q2, s.q3);
-    if (ysrc >= 0) {
-        const double x = (col + 0.5) * g.dx;                    // the (x-mapped) column the y rule is applied on
-        if (source_cell(g.side[ysrc], ysrc, g.c0, x, x, t, s)) return make_double3(s.q1, neg2 ? -s.q2 : s.q2, s.q3);
-    }
+    if (xsrc >= 0 && source_at(g, xsrc, i, r, t, s)) return make_double3(s.q1, s.q2, s.q3);
+    if (ysrc >= 0 && source_at(g, ysrc, col, r, t, s))          // col: the (x-mapped) column the y rule is applied on
+        return make_double3(s.q1, neg2 ? -s.q2 : s.q2, s.q3);
     return make_double3(c1, c2, c3);
 }
 
 // z = (q2/q1, q3/q1) of the one-deep ghost of an intermediate state, from the z of the interior cell next to the
 // edge (source step, reading A9): EXTRAP copies, REFLECT negates the normal velocity, SOURCE is analytic inside the
 // aperture and EXTRAP outside.  (PERIODIC edges never come here.)
-__device__ __noinline__ double2 ghost_z(Grid g, int sd, double along, double xc, double t, double z2, double z3) {
+__device__ __noinline__ double2 ghost_z(Grid g, int sd, int i, int r, double t, double z2, double z3) {
     const int kind = g.side[sd].kind;
     if (kind == BC_REFLECT) return sd < 2 ? make_double2(-z2, z3) : make_double2(z2, -z3);
     if (kind == BC_SOURCE) {
         Q3 s;
-        if (source_cell(g.side[sd], sd, g.c0, along, xc, t, s)) {
+        if (source_at(g, sd, i, r, t, s)) {
             const double rc = rcp_o1(s.q1);
             return make_double2(s.q2 * rc, s.q3 * rc);
         }
@@ -316,8 +313,8 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
     sts2(p + sm_off<BX>(7), F.m1, F.m2); sts2(p + sm_off<BX>(8), F.m3, F.ft1);
     // source step, x part for row ry-3
     if (th.special & 3) {
-        if (th.special & 1) zW = ghost_z(g, SIDE_XLO, (ry - 3 + 0.5) * g.dy, -0.5 * g.dx, k.t, cy.zC2, cy.zC3);
-        if (th.special & 2) zE = ghost_z(g, SIDE_XHI, (ry - 3 + 0.5) * g.dy, (g.nx + 0.5) * g.dx, k.t, cy.zC2, cy.zC3);
+        if (th.special & 1) zW = ghost_z(g, SIDE_XLO, -1, ry - 3, k.t, cy.zC2, cy.zC3);
+        if (th.special & 2) zE = ghost_z(g, SIDE_XHI, g.nx, ry - 3, k.t, cy.zC2, cy.zC3);
     }
     const double H2 = fma(k.k2, cy.zC2, fma(k.kapx, zE.x + zW.x, cy.c2));
     const double H3 = fma(k.k2, cy.zC3, fma(k.kapx, zE.y + zW.y, cy.c3));
@@ -339,10 +336,9 @@ __device__ __forceinline__ void tick(const Grid& g, const StepK& k, ThreadK& th,
     if (STEADY || R >= k.j0) {                                                // R < j1 by the loop bound
         double y2 = zN2 + cy.zS2, y3 = zN3 + cy.zS3;
         if (!STEADY && !k.py && (R == 0 || R == g.ny - 1)) {
-            const double x = (th.i + 0.5) * g.dx;
             double2 lo = make_double2(cy.zS2, cy.zS3), hi = make_double2(zN2, zN3);
-            if (R == 0) lo = ghost_z(g, SIDE_YLO, x, x, k.t, cy.zC2, cy.zC3);
-            if (R == g.ny - 1) hi = ghost_z(g, SIDE_YHI, x, x, k.t, cy.zC2, cy.zC3);
+            if (R == 0) lo = ghost_z(g, SIDE_YLO, th.i, -1, k.t, cy.zC2, cy.zC3);
+            if (R == g.ny - 1) hi = ghost_z(g, SIDE_YHI, th.i, g.ny, k.t, cy.zC2, cy.zC3);
             y2 = hi.x + lo.x; y3 = hi.y + lo.y;
         }
         const double w2 = fma(k.kapy, y2, H2), w3 = fma(k.kapy, y3, H3);

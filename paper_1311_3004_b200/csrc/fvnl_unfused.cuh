@@ -137,13 +137,13 @@ __global__ void __launch_bounds__(256) k_source_unfused(Grid g, const Clock* clk
     Q3 w, e, s, n;
     const bool px = g.side[SIDE_XLO].kind == BC_PERIODIC, py = g.side[SIDE_YLO].kind == BC_PERIODIC;
     if (i > 0) w = at(i - 1, j);
-    else w = ghost_of(g, SIDE_XLO, px ? at(g.nx - 1, j) : c, (j + 0.5) * g.dy, -0.5 * g.dx, t);
+    else w = ghost_of(g, SIDE_XLO, px ? at(g.nx - 1, j) : c, -1, j, t);
     if (i < g.nx - 1) e = at(i + 1, j);
-    else e = ghost_of(g, SIDE_XHI, px ? at(0, j) : c, (j + 0.5) * g.dy, (g.nx + 0.5) * g.dx, t);
+    else e = ghost_of(g, SIDE_XHI, px ? at(0, j) : c, g.nx, j, t);
     if (j > 0) s = at(i, j - 1);
-    else s = ghost_of(g, SIDE_YLO, py ? at(i, g.ny - 1) : c, (i + 0.5) * g.dx, (i + 0.5) * g.dx, t);
+    else s = ghost_of(g, SIDE_YLO, py ? at(i, g.ny - 1) : c, i, -1, t);
     if (j < g.ny - 1) n = at(i, j + 1);
-    else n = ghost_of(g, SIDE_YHI, py ? at(i, 0) : c, (i + 0.5) * g.dx, (i + 0.5) * g.dx, t);
+    else n = ghost_of(g, SIDE_YHI, py ? at(i, 0) : c, i, g.ny, t);
     const double rc = 1.0 / c.q1, rw = 1.0 / w.q1, re = 1.0 / e.q1, rs = 1.0 / s.q1, rn = 1.0 / n.q1;
     const double z2 = c.q2 * rc, z3 = c.q3 * rc;
     const double lx2 = (e.q2 * re + w.q2 * rw) - 2.0 * z2, ly2 = (n.q2 * rn + s.q2 * rs) - 2.0 * z2;

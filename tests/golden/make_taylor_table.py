@@ -50,7 +50,83 @@ def taylor_errors(eta, nu, threads=0, y_periodic=True):
     return E1, Einf, info
 
 
+THETAS = (0.0, np.pi / 32, np.pi / 16, np.pi / 8, np.pi / 4)
+OBLIQUE_ETAS = (5, 10, 20)
+
+
+def taylor_errors_oblique(eta, nu, theta, T=12.0, lo=-8.0, hi=22.0, half_width=2.0, threads=0):
+    """Table I rows theta_T != 0 at a size the CPU oracle can run: the profile (41) under the
+    standard rotation on the square [lo, hi]^2, analytic cells (41) on all four sides, run from t = 0 to
+    the first t_n >= T - dt/2.  E_k of (42) on q1 - 1 over the cells within 5 units of the front along the propagation
+    direction (reading A12) and within `half_width` units of the ray through the origin across it -- the paper's 10-unit
+    line, as a strip of cells.  (The paper's eta = 82, t = 100 rows need ~1e12 cell-updates: out of the oracle's reach.)"""
+    w = W.c1t_taylor(eta=eta, nu_w=nu, t_end=T, x_lo=lo, x_hi=hi, y_lo=lo, y_hi=hi, theta=theta)
+    o = Oracle(w.nx, w.ny, w.dx, w.dy, **w.medium, threads=threads)
+    for s, (k, src) in enumerate(w.bc):
+        o.set_bc(s, k, src)
+    o.set_state(*[a.numpy() for a in w.init()])
+    o.step(max(int(T * eta / nu) - 4, 1), nu, 1)
+    flags = 0
+    while o.info()["t"] < T - 0.5 * o.info()["dt"]:
+        flags |= o.step(1, nu, 1)
+    assert flags == 0
+    info = o.info()
+    q1 = o.get_state()[0]
+    x = (np.arange(w.nx) + 0.5) * w.dx + lo
+    y = (np.arange(w.ny) + 0.5) * w.dy + lo
+    X, Y = np.meshgrid(x, y)
+    ct, st = np.cos(theta), np.sin(theta)
+    xi, perp = X * ct + Y * st, -X * st + Y * ct
+    ref = W.taylor_reference(torch.from_numpy(xi), info["t"], w.extra["K"]).numpy() - 1.0
+    m = (np.abs(xi - info["t"]) <= 5.0) & (np.abs(perp) <= half_width)
+    err = np.abs((q1 - 1.0) - ref)[m]
+    return err.sum() / np.abs(ref)[m].sum(), err.max() / np.abs(ref)[m].max(), info
+
+
+def taylor_errors_moving(eta, nu, t_end=100.0, half_length=15.0, threads=0):
+    """The two-stage technique of PAPER.md:281-287 on the theta_T = 0 test: the domain [-half_length, half_length] stays
+    still until the front (at x = t) reaches its centre -- here from the start -- and then moves with it, one cell each
+    time the front has advanced by one cell; analytic cells (41) on all sides "for both stages"."""
+    w = W.c1t_taylor(eta=eta, nu_w=nu, t_end=t_end, x_lo=-half_length, x_hi=half_length, y_periodic=True)
+    o = Oracle(w.nx, w.ny, w.dx, w.dy, **w.medium, threads=threads)
+    for s, (k, src) in enumerate(w.bc):
+        o.set_bc(s, k, src)
+    o.set_state(*[a.numpy() for a in w.init()])
+    shifted = 0
+    flags = 0
+    while o.info()["t"] < t_end - 0.5 * o.info()["dt"]:
+        flags |= o.step(1, nu, 1)
+        k = int(np.floor(o.info()["t"] * eta)) - shifted          # cells the front has advanced since the last move
+        if k > 0:
+            o.shift(k)
+            shifted += k
+    assert flags == 0
+    info = o.info()
+    q1 = o.get_state()[0][1]
+    x = (np.arange(w.nx) + 0.5) * w.dx - half_length + shifted * w.dx
+    ref = W.taylor_reference(torch.from_numpy(x), info["t"], w.extra["K"]).numpy() - 1.0
+    m = np.abs(x - info["t"]) <= 5.0
+    err = np.abs((q1 - 1.0) - ref)[m]
+    return err.sum() / np.abs(ref)[m].sum(), err.max() / np.abs(ref)[m].max(), info, shifted
+
+
+def write_oblique_table():
+    out = os.path.join(os.path.dirname(os.path.abspath(__file__)), "taylor_oblique_oracle.txt")
+    lines = ["# written by tests/golden/make_taylor_table.py --oblique (oracle only).  Taylor profile (41) at an angle theta_T on",
+             "# [-8, 22]^2, nu_W = 0.9, t = 12 (taylor_errors_oblique).  columns: eta theta_T E1 Einf t_final steps"]
+    for eta in OBLIQUE_ETAS:
+        for th in THETAS:
+            E1, Einf, info = taylor_errors_oblique(eta, 0.9, th)
+            lines.append(f"{eta} {th!r} {E1:.6e} {Einf:.6e} {info['t']:.12f} {info['steps']}")
+            print(lines[-1], flush=True)
+    with open(out, "w") as f:
+        f.write("\n".join(lines) + "\n")
+
+
 if __name__ == "__main__":
+    if "--oblique" in sys.argv:
+        write_oblique_table()
+        sys.exit(0)
     out = os.path.join(os.path.dirname(os.path.abspath(__file__)), "taylor_table_oracle.txt")
     lines = ["# written by tests/golden/make_taylor_table.py (oracle only). columns: eta nu_W E1 Einf t_final steps last_cfl"]
     for eta in ETAS:

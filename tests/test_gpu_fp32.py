@@ -168,3 +168,22 @@ def test_fp32_c5_16384_windows():
         print(f"PARITY32 C5-{n} window ({i0},{j0}) {wx}x{wy} steps=100 err={err:.3e} tol={TOL32:g}")
         worst = max(worst, err)
     assert worst <= TOL32
+
+
+def test_fp32_oblique_taylor_and_moving_domain():
+    """The two other 'next' rows in fp32: oblique Taylor shock and the moving domain."""
+    import math
+    w = W.c1t_taylor(eta=10, nu_w=0.9, x_lo=-4.0, x_hi=10.0, y_lo=-5.0, y_hi=8.0, theta=math.pi / 8)
+    check32(w, steps=90, metric=parity_error_global)
+    w = W.c2_pulse(n=260, ny=90, sigma_cells=6.0, steps=1, amp=1e-3)
+    state = [a.numpy().copy() for a in w.init()]
+    o = oracle_from_workload(w, threads=0, state=state)
+    s = solver_from_workload(w, state=[torch.from_numpy(a) for a in state], precision=32)
+    for n, k in ((7, 1), (5, 3), (11, 2), (9, 1)):
+        assert o.step(n, 0.9, 1) == 0 and s.step(n, 0.9, 1) == 0
+        o.shift(k)
+        s.shift(k)
+    assert o.step(6, 0.9, 1) == 0 and s.step(6, 0.9, 1) == 0
+    err = parity_error([a.cpu().numpy() for a in s.get_state(as_q64=True)], o.get_state())
+    print(f"PARITY32 moving pulse err={err:.3e}")
+    assert err <= TOL32

@@ -564,3 +564,55 @@ def test_sources_on_every_side(kernel):
     cases.append(w)
     for w in cases:
         check(w, kernel=kernel)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
+def test_oblique_taylor_shocks(kernel):
+    """the profile (41) propagating at theta_T = pi/8 and pi/4 on a 2-D grid, analytic cells
+    (41) on all four sides (both sweeps, the splitting and every edge kernel path at once).  Perturbation 1e-7 on a unit
+    background: bar 1e-7 on one scale for all fields, as for C1-T."""
+    import math
+    for theta in (math.pi / 8, math.pi / 4):
+        w = W.c1t_taylor(eta=10, nu_w=0.9, x_lo=-4.0, x_hi=10.0, y_lo=-5.0, y_hi=8.0, theta=theta)
+        check(w, steps=90, tol=1e-7, metric=parity_error_global, kernel=kernel)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
+def test_moving_domain(kernel):
+    """the domain moves with the wave (fvnl_shift).  (a) a pulse under extrapolation
+    edges, the domain moved by 1..3 cells every few steps; (b) the Taylor test with analytic cells (41) entering on the
+    right, moved one cell whenever the front has advanced by one, as the oracle's driver does."""
+    w = W.c2_pulse(n=260, ny=90, sigma_cells=6.0, steps=1, amp=1e-3)
+    state = [a.numpy().copy() for a in w.init()]
+    o = oracle_from_workload(w, threads=0, state=state)
+    s = solver_from_workload(w, state=[torch.from_numpy(a) for a in state])
+    select(s, kernel)
+    for n, k in ((7, 1), (5, 3), (11, 2), (4, 0), (9, 1)):
+        assert o.step(n, 0.9, 1) == 0 and s.step(n, 0.9, 1) == 0
+        o.shift(k)
+        s.shift(k)
+    assert o.step(6, 0.9, 1) == 0 and s.step(6, 0.9, 1) == 0
+    assert s.info()["t"] == pytest.approx(o.info()["t"], rel=1e-12)
+    err = parity_error([a.cpu().numpy() for a in s.get_state()], o.get_state())
+    print(f"PARITY moving pulse kernel={kernel} err={err:.3e}")
+    assert err <= TOL
+    tw = W.c1t_taylor(eta=10, nu_w=0.9, x_lo=-6.0, x_hi=6.0, ny=6, y_periodic=False)
+    state = [a.numpy().copy() for a in tw.init()]
+    o = oracle_from_workload(tw, threads=0, state=state)
+    s = solver_from_workload(tw, state=[torch.from_numpy(a) for a in state])
+    select(s, kernel)
+    shifted = 0
+    for _ in range(120):
+        assert o.step(1, 0.9, 1) == 0 and s.step(1, 0.9, 1) == 0
+        k = int(np.floor(o.info()["t"] * 10)) - shifted
+        if k > 0:
+            o.shift(k)
+            s.shift(k)
+            shifted += k
+    assert shifted >= 100
+    err = parity_error_global([a.cpu().numpy() for a in s.get_state()], o.get_state())
+    print(f"PARITY moving Taylor kernel={kernel} shifted={shifted} err={err:.3e}")
+    assert err <= 1e-7
+    import paper_1311_3004_b200 as P
+    with pytest.raises(P.FvnlError):
+        solver_from_workload(W.c3_random(n=16, ny=16)).shift(1)

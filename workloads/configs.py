@@ -26,9 +26,9 @@ LAMBDA_1MHZ = 1500.0 / 1.0e6          # 1.5 mm
 TAYLOR_STEEP = 2.0 * math.atanh(0.8)
 
 
-def _src(shape, amp, freq_hz=0.0, focus_m=0.0, centre_m=0.0, half_aperture_m=0.0, t0_s=0.0, steep=0.0):
+def _src(shape, amp, freq_hz=0.0, focus_m=0.0, centre_m=0.0, half_aperture_m=0.0, t0_s=0.0, steep=0.0, theta=0.0):
     return dict(shape=shape, amp=amp, freq_hz=freq_hz, focus_m=focus_m, centre_m=centre_m,
-                half_aperture_m=half_aperture_m, t0_s=t0_s, steep=steep)
+                half_aperture_m=half_aperture_m, t0_s=t0_s, steep=steep, theta=theta)
 
 
 @dataclass
@@ -76,24 +76,32 @@ def taylor_reference(x, t, K=1.0e-7, steep=TAYLOR_STEEP):
 
 
 def c1t_taylor(eta=20, nu_w=0.9, t_end=100.0, ny=4, x_lo=-15.0, x_hi=115.0, K=1.0e-7, beta=3.5,
-               y_periodic=False) -> Workload:
-    """C1-T: the paper's own Taylor-shock test, theta_T = 0.  Dimensionless: c0 = rho0 = 1,
-    dx = 1/eta, delta~ = K beta / steep (the Taylor balance for tanh(steep (x-t)) of amplitude K)."""
+               y_periodic=False, theta=0.0, y_lo=0.0, y_hi=None) -> Workload:
+    """C1-T: the paper's own Taylor-shock test.  Dimensionless: c0 = rho0 = 1, dx = 1/eta,
+    delta~ = K beta / steep (the Taylor balance for tanh(steep (x-t)) of amplitude K).
+    theta = theta_T, the propagation angle from the x_1 axis: the profile (41) under the standard rotation,
+    q1 = 1 - K tanh(steep (x cos(theta) + y sin(theta) - t)), (q2, q3) = (q1 - 1)(cos(theta), sin(theta)), on a 2-D grid
+    x in [x_lo, x_hi], y in [y_lo, y_hi] (y_hi = None: ny rows), analytic cells (41) on all four sides."""
     nx = int(round((x_hi - x_lo) * eta))
     dx = 1.0 / eta
+    if y_hi is not None:
+        ny = int(round((y_hi - y_lo) * eta))
     med = dict(c0=1.0, rho0=1.0, beta=beta, delta=K * beta / TAYLOR_STEEP)
-    # x of fvnl_source TANH is measured from the x-lo edge: x_phys = x_edge + x_lo -> t0 = -x_lo / c0
-    src = _src(TANH, amp=K, t0_s=-x_lo, steep=TAYLOR_STEEP)
+    ct, st = math.cos(theta), math.sin(theta)
+    # x, y of fvnl_source TANH are measured from the x-lo / y-lo edge: xi_phys = xi_edge + (x_lo ct + y_lo st) -> t0
+    src = _src(TANH, amp=K, t0_s=-(x_lo * ct + y_lo * st), steep=TAYLOR_STEEP, theta=theta)
     ysides = (PERIODIC, None) if y_periodic else (SOURCE, dict(src))
 
     def init(device="cpu"):
         x = (torch.arange(nx, dtype=torch.float64, device=device) + 0.5) * dx + x_lo
-        q1 = taylor_reference(x, 0.0, K).expand(ny, nx).contiguous()
-        return q1, q1 - 1.0, torch.zeros_like(q1)
+        y = (torch.arange(ny, dtype=torch.float64, device=device) + 0.5) * dx + y_lo
+        xi = x[None, :] * ct + y[:, None] * st
+        q1 = taylor_reference(xi, 0.0, K).contiguous()
+        return q1, (q1 - 1.0) * ct, (q1 - 1.0) * st + 0.0
 
-    return Workload(f"C1-T(eta={eta},nu={nu_w})", nx, ny, dx, dx, med,
+    return Workload(f"C1-T(eta={eta},nu={nu_w},theta={theta:.4f})" if theta else f"C1-T(eta={eta},nu={nu_w})", nx, ny, dx, dx, med,
                     [(SOURCE, dict(src)), (SOURCE, dict(src)), ysides, ysides], 1, nu_w, 0, init,
-                    "run until t >= t_end", extra=dict(t_end=t_end, x_lo=x_lo, K=K, eta=eta))
+                    "run until t >= t_end", extra=dict(t_end=t_end, x_lo=x_lo, y_lo=y_lo, K=K, eta=eta, theta=theta))
 
 
 def c2_pulse(n=1024, steps=500, sigma_cells=20.0, amp=1.0e-3, nu_w=0.9, ny=None) -> Workload:
@@ -150,7 +158,7 @@ def c3_random(n=4096, steps=200, nu_w=0.8, seed=1311300403, ny=None, name="C3", 
     nx, ny = n, (n if ny is None else ny)
     dx = LAMBDA_1MHZ / 32
     return Workload(name, nx, ny, dx, dx, dict(MEDIUM_WATER), [(PERIODIC, None)] * 4, 1, nu_w, steps,
-                    _multi_gaussian(nx, ny, seed, c0=MEDIUM_WATER["c0"], **kw), f"seed {seed}")
+                    _multi_gaussian(nx, ny, seed, c0=MEDIUM_WATER["c0"], **kw), f"seed {seed}", extra=dict(seed=seed))
 
 
 def c5_sweep(n=16384, steps=100, nu_w=0.9, ny=None) -> Workload:
