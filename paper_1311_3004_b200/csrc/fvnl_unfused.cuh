@@ -65,69 +65,45 @@ __device__ __forceinline__ Q3 sweep_cell(const CellX c[5], double lam, double be
     return o;
 }
 
-// O2: x-sweep (24) of the y-extended mesh, rows -2 .. ny+1 -> star (row r stored at r+2).  grid.y = ny+4.
-__global__ void __launch_bounds__(256) k_xsweep_unfused(Grid g, Clock* clk, const double* __restrict__ q1,
-                                                        const double* __restrict__ q2, const double* __restrict__ q3,
-                                                        double* __restrict__ s1, double* __restrict__ s2,
-                                                        double* __restrict__ s3) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int r = (int)blockIdx.y - 2;
-    const double t = clk->t, lam = clk->lamx;
-    int flags = 0;
-    double smax = 0.0;
-    if (i < g.nx) {
-        CellX c[5];
+// ---- one cell of each sub-step ---------------------------------------------------------------------------------------
+// O2: Q*(i, r) of the x-sweep (24) on the y-extended mesh (row r in -2 .. ny+1 is stored at r + 2 of star).
+__device__ __forceinline__ void xsweep_cell(const Grid& g, double t, double lam, const double* q1, const double* q2,
+                                            const double* q3, double* s1, double* s2, double* s3, int i, int r, double& smax,
+                                            int& flags) {
+    CellX c[5];
+    int f = 0;
 #pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            const Q3 q = load_ext(g, q1, q2, q3, i - 2 + k, r, t);
-            c[k] = make_cell(q.q1, q.q2, q.q3, flags);
-        }
-        double sl, sr;
-        const Q3 o = sweep_cell(c, lam, 2.0 * (g.beta - 1.0), sl, sr, flags);
-        const size_t idx = (size_t)(r + 2) * g.nx + i;
-        s1[idx] = o.q1; s2[idx] = o.q2; s3[idx] = o.q3;
-        if (r >= 0 && r < g.ny) smax = fmax(sl, sr); else flags = 0;      // ghost rows do not enter M (O5)
+    for (int k = 0; k < 5; ++k) {
+        const Q3 q = load_ext(g, q1, q2, q3, i - 2 + k, r, t);
+        c[k] = make_cell(q.q1, q.q2, q.q3, f);
     }
-    block_max_to(&clk->sx_bits, smax);
-    block_flags_to(&clk->flags, flags);
+    double sl, sr;
+    const Q3 o = sweep_cell(c, lam, 2.0 * (g.beta - 1.0), sl, sr, f);
+    const size_t idx = (size_t)(r + 2) * g.nx + i;
+    s1[idx] = o.q1; s2[idx] = o.q2; s3[idx] = o.q3;
+    if (r >= 0 && r < g.ny) { smax = fmax(smax, fmax(sl, sr)); flags |= f; }      // ghost rows do not enter M (O5)
 }
 
-// O3: y-sweep (25) of star with positions 2 and 3 switched -> o1..o3 (interior).
-__global__ void __launch_bounds__(256) k_ysweep_unfused(Grid g, Clock* clk, const double* __restrict__ s1,
-                                                        const double* __restrict__ s2, const double* __restrict__ s3,
-                                                        double* __restrict__ o1, double* __restrict__ o2,
-                                                        double* __restrict__ o3) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y;
-    const double lam = clk->lamy;
-    int flags = 0;
-    double smax = 0.0;
-    if (i < g.nx) {
-        CellX c[5];
+// O3: Q**(i, j) of the y-sweep (25) of star with positions 2 and 3 switched.
+__device__ __forceinline__ void ysweep_cell(const Grid& g, double lam, const double* s1, const double* s2, const double* s3,
+                                            double* o1, double* o2, double* o3, int i, int j, double& smax, int& flags) {
+    CellX c[5];
 #pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            const size_t idx = (size_t)(j + k) * g.nx + i;               // star row (j-2+k) is stored at j+k
-            c[k] = make_cell(s1[idx], s3[idx], s2[idx], flags);
-        }
-        double sl, sr;
-        const Q3 o = sweep_cell(c, lam, 2.0 * (g.beta - 1.0), sl, sr, flags);
-        const size_t idx = (size_t)j * g.nx + i;
-        o1[idx] = o.q1; o2[idx] = o.q3; o3[idx] = o.q2;
-        smax = fmax(sl, sr);
+    for (int k = 0; k < 5; ++k) {
+        const size_t idx = (size_t)(j + k) * g.nx + i;               // star row (j-2+k) is stored at j+k
+        c[k] = make_cell(s1[idx], s3[idx], s2[idx], flags);
     }
-    block_max_to(&clk->sy_bits, smax);
-    block_flags_to(&clk->flags, flags);
+    double sl, sr;
+    const Q3 o = sweep_cell(c, lam, 2.0 * (g.beta - 1.0), sl, sr, flags);
+    const size_t idx = (size_t)j * g.nx + i;
+    o1[idx] = o.q1; o2[idx] = o.q3; o3[idx] = o.q2;
+    smax = fmax(smax, fmax(sl, sr));
 }
 
 // O4: source step (26): q^m += kap_x d2x(q^m/q^1) + kap_y d2y(q^m/q^1), m = 2, 3 (readings A1, A2).
-__global__ void __launch_bounds__(256) k_source_unfused(Grid g, const Clock* clk, const double* __restrict__ a1,
-                                                        const double* __restrict__ a2, const double* __restrict__ a3,
-                                                        double* __restrict__ o1, double* __restrict__ o2,
-                                                        double* __restrict__ o3) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y;
-    if (i >= g.nx) return;
-    const double t = clk->t, kx = clk->kapx, ky = clk->kapy;
+__device__ __forceinline__ void source_step_cell(const Grid& g, double t, double kx, double ky, const double* a1,
+                                                 const double* a2, const double* a3, double* o1, double* o2, double* o3,
+                                                 int i, int j) {
     auto at = [&](int ii, int jj) {
         const size_t idx = (size_t)jj * g.nx + ii;
         Q3 c; c.q1 = a1[idx]; c.q2 = a2[idx]; c.q3 = a3[idx];
@@ -152,6 +128,40 @@ __global__ void __launch_bounds__(256) k_source_unfused(Grid g, const Clock* clk
     o1[idx] = c.q1;
     o2[idx] = fma(ky, ly2, fma(kx, lx2, c.q2));
     o3[idx] = fma(ky, ly3, fma(kx, lx3, c.q3));
+}
+
+// O2 as a kernel.  grid.y = ny+4.
+__global__ void __launch_bounds__(256) k_xsweep_unfused(Grid g, Clock* clk, const double* __restrict__ q1,
+                                                        const double* __restrict__ q2, const double* __restrict__ q3,
+                                                        double* __restrict__ s1, double* __restrict__ s2,
+                                                        double* __restrict__ s3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = (int)blockIdx.y - 2;
+    int flags = 0;
+    double smax = 0.0;
+    if (i < g.nx) xsweep_cell(g, clk->t, clk->lamx, q1, q2, q3, s1, s2, s3, i, r, smax, flags);
+    block_max_to(&clk->sx_bits, smax);
+    block_flags_to(&clk->flags, flags);
+}
+
+__global__ void __launch_bounds__(256) k_ysweep_unfused(Grid g, Clock* clk, const double* __restrict__ s1,
+                                                        const double* __restrict__ s2, const double* __restrict__ s3,
+                                                        double* __restrict__ o1, double* __restrict__ o2,
+                                                        double* __restrict__ o3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int flags = 0;
+    double smax = 0.0;
+    if (i < g.nx) ysweep_cell(g, clk->lamy, s1, s2, s3, o1, o2, o3, i, blockIdx.y, smax, flags);
+    block_max_to(&clk->sy_bits, smax);
+    block_flags_to(&clk->flags, flags);
+}
+
+__global__ void __launch_bounds__(256) k_source_unfused(Grid g, const Clock* clk, const double* __restrict__ a1,
+                                                        const double* __restrict__ a2, const double* __restrict__ a3,
+                                                        double* __restrict__ o1, double* __restrict__ o2,
+                                                        double* __restrict__ o3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < g.nx) source_step_cell(g, clk->t, clk->kapx, clk->kapy, a1, a2, a3, o1, o2, o3, i, blockIdx.y);
 }
 
 }  // namespace fvnl
