@@ -48,7 +48,15 @@ template <class T> struct XThreadT {
     T rn1, rn2;                              // and their 1/(r.r)
     CxT<T> cx;                               // this column's cell of the row converted in the previous tick
     T aq[2][3];                              // Q^n(i, .) of the rows loaded in the previous two ticks, by row parity
-};
+    const double* srow;                      // ghost column of a SOURCE x-side: its records of this step (record of row r at
+    double s1, s2, s3;                       // srow + 3 r), and the record of the row phase A converts NEXT, loaded one tick
+};                                           // ahead (an L2 round trip inside the tick stalls the whole warp)
+
+// The analytic record of row r for a ghost column of a SOURCE x-side (q1 <= 0: none / outside the aperture).
+template <class T> __device__ __forceinline__ void x_prefetch_source(const Grid& g, XThreadT<T>& th, int r) {
+    if (th.srow && r >= -3 && r <= g.ny + 2) { const double* sp = th.srow + 3 * r; th.s1 = sp[0]; th.s2 = sp[1]; th.s3 = sp[2]; }
+    else th.s1 = -1.0;
+}
 
 // Density variable of a cell from a full-form fp64 value (analytic ghost cells): q1, or rho' = q1 - 1 in fp32.
 template <class T> __device__ __forceinline__ T dens_var(double q1) { return Num<T>::perturbation ? T(q1 - 1.0) : T(q1); }
@@ -132,12 +140,9 @@ __device__ __forceinline__ void ws_xtick(const Grid& g, const StepKT<T>& k, XThr
             if (!STEADY && rm.neg3) a3 = -a3;
             if (th.special & 4) a2 = -a2;
             bool done = false;                                                // x rule first, then y rule (as load_mapped)
-            if ((th.special & 8) && r >= -3 && r <= g.ny + 2) {
-                const int sd = th.cm.xsrc, l = sd == SIDE_XLO ? -1 - th.i : th.i - g.nx;
-                if (l < 3) {
-                    const double* sp = k.src + src_off(g.nx, g.ny, sd) + 3 * ((size_t)(g.ny + 6) * l + r + 3);
-                    if (sp[0] > 0.0) { a1 = dens_var<T>(sp[0]); a2 = T(sp[1]); a3 = T(sp[2]); done = true; }
-                }
+            if (th.special & 8) {                                             // record loaded in the previous tick
+                if (th.s1 > 0.0) { a1 = dens_var<T>(th.s1); a2 = T(th.s2); a3 = T(th.s3); done = true; }
+                x_prefetch_source(g, th, r + 1);
             }
             if (!STEADY && !done && rm.ysrc >= 0) {
                 const int sd = rm.ysrc, l = sd == SIDE_YLO ? -1 - r : r - g.ny;
@@ -181,7 +186,25 @@ template <class T> struct YThreadT {
     char* p;
     T smy;
     int mqy, mdy, mxo;
+    const double* grow;                      // edge column next to a SOURCE x-side: layer-0 records of that side (row m at
+    double g1, g2, g3;                       // grow + 3 m), and the record the NEXT tick's source step needs, loaded ahead
 };
+
+template <class T> __device__ __forceinline__ void y_prefetch_source(const Grid& g, YThreadT<T>& th, int m) {
+    if (th.grow) { m = min(max(m, -3), g.ny + 2); const double* sp = th.grow + 3 * m; th.g1 = sp[0]; th.g2 = sp[1]; th.g3 = sp[2]; }
+}
+
+// z of the one-deep ghost of Q** at an x edge from the record loaded ahead (y_prefetch_source), else by the plain rule.
+template <class T>
+__device__ __forceinline__ typename Num<T>::T2 ghost_z_x(const Grid& g, const YThreadT<T>& th, int sd, T z2, T z3) {
+    const int kind = g.side[sd].kind;
+    if (kind == BC_REFLECT) return Num<T>::make2(-z2, z3);
+    if (kind == BC_SOURCE && th.g1 > 0.0) {
+        const double rc = rcp_o1(th.g1);
+        return Num<T>::make2(T(th.g2 * rc), T(th.g3 * rc));
+    }
+    return Num<T>::make2(z2, z3);
+}
 
 template <class T> struct YCarryT {
     T gp1, gp2, gp3, gf1;                    // right-going part (and F~, comp. 1) of the y-interface below B
@@ -219,9 +242,10 @@ __device__ __forceinline__ void ws_ytick(const Grid& g, const StepKT<T>& k, YThr
     cy.gp1 = G.p1; cy.gp2 = G.p2; cy.gp3 = G.p3; cy.gf1 = G.ft1;
     cy.q1 = N.c.q1; cy.q2 = N.c.q2; cy.q3 = N.c.q3;                           // Q*(ry-3), y-form: next tick's lower row
     auto zW = ldp<T>(p + ws_arr2<T>(11, R) - E), zE = ldp<T>(p + ws_arr2<T>(11, R) + E);   // z of row ry-5, published last tick
-    if (th.special & 3) {
-        if (th.special & 1) zW = ghost_z_plain<T>(g, k.src, SIDE_XLO, ry - 5, cy.zC2, cy.zC3);
-        if (th.special & 2) zE = ghost_z_plain<T>(g, k.src, SIDE_XHI, ry - 5, cy.zC2, cy.zC3);
+    if (th.special & 3) {                                                     // (record of row ry-5 loaded in the previous tick)
+        if (th.special & 1) zW = ghost_z_x<T>(g, th, SIDE_XLO, cy.zC2, cy.zC3);
+        if (th.special & 2) zE = ghost_z_x<T>(g, th, SIDE_XHI, cy.zC2, cy.zC3);
+        y_prefetch_source(g, th, ry - 4);
     }
     const T H2 = fma(k.k2, cy.zC2, fma(k.kapx, zE.x + zW.x, cy.c2));
     const T H3 = fma(k.k2, cy.zC3, fma(k.kapx, zE.y + zW.y, cy.c3));
@@ -328,6 +352,12 @@ k_step_ws(Grid g, Clock* clk, const T* __restrict__ q1, const T* __restrict__ q2
         th.rn1 = th.rn2 = T(0.5);
         th.cx = {eq1, T(0), T(0), T(0), T(0)};
         for (int d = 0; d < 2; ++d) th.aq[d][0] = eq1, th.aq[d][1] = th.aq[d][2] = T(0);
+        th.srow = nullptr;
+        if (th.cm.xsrc >= 0) {
+            const int l = th.cm.xsrc == SIDE_XLO ? -1 - i : i - g.nx;
+            if (l < 3) th.srow = k.src + src_off(g.nx, g.ny, th.cm.xsrc) + 3 * ((size_t)(g.ny + 6) * l + 3);
+        }
+        x_prefetch_source(g, th, r0);                              // the first row phase A converts
         for (int d = 0; d < 2; ++d) {                              // rows r0 and r0+1 start their way into the ring
             const RowMap rm = map_row(g, r0 + d);
             const size_t idx = (size_t)rm.row * g.nx + th.cm.col;
@@ -367,6 +397,12 @@ k_step_ws(Grid g, Clock* clk, const T* __restrict__ q1, const T* __restrict__ q2
         th.out_col = c >= 3 && c <= WS_COLS - 4 && i >= 0 && i < g.nx;
         th.p = smem + (c + 1) * ws_elem<T>();
         th.smy = T(0); th.mqy = th.mdy = 0x7fffffff; th.mxo = 0;
+        th.grow = nullptr; th.g1 = -1.0; th.g2 = th.g3 = 0.0;
+        if (th.special & 3) {
+            const int sd = (th.special & 1) ? SIDE_XLO : SIDE_XHI;             // (nx >= 4: a column is next to one x edge only)
+            if (g.side[sd].kind == BC_SOURCE) th.grow = k.src + src_off(g.nx, g.ny, sd) + 3 * 3;
+        }
+        y_prefetch_source(g, th, r0 - 1 - 5);                                  // row of the first tick's source step
         YSetT<T> Y0, Y1;
         Y0.c = {eq1, T(0), T(0), T(0), T(0)};
         Y0.w = {T(0), T(1), T(0), T(0), T(-1), T(0), T(0), T(0)};
