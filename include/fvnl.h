@@ -171,8 +171,13 @@ int fvnl_get_info(fvnl_ctx* ctx, double* t_s, double* last_dt_s, double* last_cf
  * FVNL_OPT_VARIANT (one-pass kernel): 0 = warp-specialised kernel k_step_ws (default), 1 = single-role kernel
  *   k_step_fused (one thread does both sweeps of its column; evaluates analytic edge cells in place).
  * FVNL_OPT_ROWS_PER_BLOCK: rows one thread block of the one-pass kernel marches over (0 = automatic).
- * FVNL_OPT_KERNEL_TIMING: see fvnl_get_kernel_time. */
-enum { FVNL_OPT_KERNEL = 0, FVNL_OPT_ROWS_PER_BLOCK = 1, FVNL_OPT_KERNEL_TIMING = 2, FVNL_OPT_VARIANT = 3 };
+ * FVNL_OPT_KERNEL_TIMING: see fvnl_get_kernel_time.
+ * FVNL_OPT_SMALL_GRID: 1 (default) = a double-precision grid of at most 16384 cells runs ALL steps of a fvnl_step call in
+ *   one launch of one thread-block cluster (up to 16 CTAs; the time loop, the CFL clock and the analytic edge cells inside
+ *   the kernel) instead of one launch per step -- such grids are bound by launches and latency (C1: 512 x 4 cells);
+ *   0 = always one launch per step.  Ignored while FVNL_OPT_KERNEL_TIMING is on or another kernel / variant is selected. */
+enum { FVNL_OPT_KERNEL = 0, FVNL_OPT_ROWS_PER_BLOCK = 1, FVNL_OPT_KERNEL_TIMING = 2, FVNL_OPT_VARIANT = 3,
+       FVNL_OPT_SMALL_GRID = 4 };
 enum { FVNL_KERNEL_DEFAULT = 0, FVNL_KERNEL_UNFUSED = 1 };
 int fvnl_set_option(fvnl_ctx* ctx, int option, int value);
 

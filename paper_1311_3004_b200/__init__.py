@@ -25,7 +25,7 @@ SINE, PACKET, TANH = 0, 1, 2
 XLO, XHI, YLO, YHI = 0, 1, 2, 3
 OK, EARG, EALLOC, ECUDA, ESTATE = 0, 1, 2, 3, 4
 ECFL, ENONREAL, ENONPOS, ENAN = 16, 32, 64, 128
-OPT_KERNEL, OPT_ROWS_PER_BLOCK, OPT_KERNEL_TIMING, OPT_VARIANT = 0, 1, 2, 3
+OPT_KERNEL, OPT_ROWS_PER_BLOCK, OPT_KERNEL_TIMING, OPT_VARIANT, OPT_SMALL_GRID = 0, 1, 2, 3, 4
 TIMED_STEP, TIMED_XSWEEP, TIMED_YSWEEP, TIMED_SOURCE = 0, 1, 2, 3
 KERNEL_DEFAULT, KERNEL_UNFUSED = 0, 1
 ON_HOST, ON_DEVICE, PLANES_F64 = 0, 1, 2

@@ -12,6 +12,7 @@
 
 #include "../../include/fvnl.h"
 #include "fvnl_ws.cuh"
+#include "fvnl_small.cuh"
 
 using namespace fvnl;
 
@@ -166,6 +167,9 @@ struct fvnl_ctx {
     int kernel;                 // FVNL_KERNEL_*
     int rows_per_block;         // fused kernel: rows per chunk (0 = automatic)
     int variant;                // fused kernel: launch variant
+    int small;                  // FVNL_OPT_SMALL_GRID: 1 = grids of at most SMALL_MAX_CELLS cells run all steps of a call in one
+                                // cluster launch (k_steps_cluster), 0 = never
+    int small_cluster;          // CTAs per cluster the device accepts for it (0 = not probed yet, -1 = unavailable)
     long launches;
     // CUDA graph of two consecutive steps (state A -> B -> A), for grids so small that launches dominate
     cudaStream_t gstream;       // capture stream (never executes anything)
@@ -286,6 +290,7 @@ extern "C" int fvnl_create(fvnl_ctx** out, int nx, int ny, double dx, double dy,
     c->need_prepass = true;
     c->kernel = FVNL_KERNEL_DEFAULT;
     c->variant = DEFAULT_VARIANT;
+    c->small = 1;
     // per device (function attributes belong to the context of the current device)
     ok = ok && cudaFuncSetAttribute(k_step_ws<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, ws_smem_bytes<double>()) == cudaSuccess;
     ok = ok && cudaFuncSetAttribute(k_step_ws<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, ws_smem_bytes<float>()) == cudaSuccess;
@@ -348,6 +353,11 @@ extern "C" int fvnl_set_option(fvnl_ctx* c, int option, int value) {
     }
     if (option == FVNL_OPT_KERNEL_TIMING) {
         c->timing = value != 0;
+        return FVNL_OK;
+    }
+    if (option == FVNL_OPT_SMALL_GRID) {
+        if (value != 0 && value != 1) return FVNL_EARG;
+        c->small = value;
         return FVNL_OK;
     }
     return FVNL_EARG;
@@ -499,6 +509,58 @@ static void onepass_step(fvnl_ctx* c, double value, int mode, int more) {
     c->launches += 1;
 }
 
+// Small grids: all `nsteps` steps in one launch of one thread-block cluster (fvnl_small.cuh).  Returns false when the
+// device does not take such a launch (the caller then runs the per-step path).
+static void small_config(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* at, const fvnl_ctx* c, int cs) {
+    *cfg = cudaLaunchConfig_t{};
+    cfg->gridDim = dim3(cs); cfg->blockDim = dim3(SMALL_THREADS + 32); cfg->stream = c->stream;
+    cfg->dynamicSmemBytes = small_smem_bytes(c->g.nx, c->g.ny, cs);
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg->attrs = at; cfg->numAttrs = 1;
+}
+
+// CTAs of the cluster: the smallest power of two that gives every cell of the largest sub-step a thread of its own, up to
+// the largest cluster the device schedules (16 = non-portable size, else 8) with the shared memory the state then needs.
+static int small_cluster_size(fvnl_ctx* c) {
+    if (c->small_cluster != 0) return c->small_cluster > 0 ? c->small_cluster : 0;
+    c->small_cluster = -1;
+    (void)cudaFuncSetAttribute(k_steps_cluster, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    (void)cudaFuncSetAttribute(k_steps_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    (void)cudaGetLastError();
+    int want = 1;
+    while (want < SMALL_MAX_CLUSTER && want * SMALL_THREADS < c->g.nx * (c->g.ny + 4)) want *= 2;
+    for (int cs = want; cs >= 1; cs /= 2) {
+        if (small_smem_bytes(c->g.nx, c->g.ny, cs) > 200 * 1024) break;
+        cudaLaunchConfig_t cfg;
+        cudaLaunchAttribute at[1];
+        small_config(&cfg, at, c, cs);
+        int ncl = 0;
+        if (cudaOccupancyMaxActiveClusters(&ncl, k_steps_cluster, &cfg) == cudaSuccess && ncl >= 1) { c->small_cluster = cs; break; }
+        (void)cudaGetLastError();
+    }
+    return c->small_cluster > 0 ? c->small_cluster : 0;
+}
+
+static bool small_steps(fvnl_ctx* c, long nsteps, double value, int mode) {
+    const int cs = small_cluster_size(c);
+    if (cs < 1) return false;
+    int logc = 0;
+    while ((1 << logc) < cs) ++logc;
+    double** q = (double**)c->buf[c->cur];
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute at[1];
+    small_config(&cfg, at, c, cs);
+    if (cudaLaunchKernelEx(&cfg, k_steps_cluster, c->g, c->clk, q[0], q[1], q[2], logc, (long long)nsteps, value, mode) !=
+        cudaSuccess) {
+        (void)cudaGetLastError();
+        c->small_cluster = -1;
+        return false;
+    }
+    c->launches += 1;                                               // the state stays in buf[cur]
+    return true;
+}
+
 extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
     if (!c || nsteps < 0 || !(value > 0.0) || (mode != 0 && mode != 1)) return FVNL_EARG;
     if (!c->have_state) return FVNL_ESTATE;
@@ -528,9 +590,13 @@ extern "C" int fvnl_step(fvnl_ctx* c, long nsteps, double value, int mode) {
         if (rc) return rc;
     }
     long n = 0;
+    // Small grids: one cluster launch for the whole call.
+    if (c->small && c->kernel == FVNL_KERNEL_DEFAULT && c->variant == DEFAULT_VARIANT && c->prec == 64 && !c->timing &&
+        c->n <= SMALL_MAX_CELLS && small_steps(c, nsteps, value, mode))
+        n = nsteps;
     // Launch-bound grids: replay a captured graph of two steps (A -> B -> A) while at least three steps remain; the last
     // steps (the final one computes no dt for a successor) go out as plain launches below.
-    if (c->kernel == FVNL_KERNEL_DEFAULT && !c->timing && c->n <= GRAPH_MAX_CELLS && nsteps >= 4) {
+    if (n == 0 && c->kernel == FVNL_KERNEL_DEFAULT && !c->timing && c->n <= GRAPH_MAX_CELLS && nsteps >= 4) {
         if (!c->gvalid || c->gvalue != value || c->gmode != mode || c->gcur != c->cur || c->gvariant != c->variant ||
             c->grows != c->rows_per_block) {
             if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }

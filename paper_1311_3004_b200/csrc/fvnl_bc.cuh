@@ -186,8 +186,9 @@ __device__ __forceinline__ int clampi(int i, int n) { return i < 0 ? 0 : (i >= n
 // Value of the ghost-extended mesh at column i, row r (any integers; the rules are exact for the two ghost
 // layers the scheme uses and merely safe beyond them).  The x rule is applied on the y-extended rows, i.e. a
 // corner cell is the x-ghost of a y-ghost row (reading A9).  `t` = t_n.
-__device__ __forceinline__ Q3 load_ext(const Grid& g, const double* __restrict__ q1, const double* __restrict__ q2,
-                                       const double* __restrict__ q3, int i, int r, double t) {
+// `cells`: where the interior cells live -- any callable idx -> Q3 (idx = row * nx + column).
+template <class Cells>
+__device__ __forceinline__ Q3 load_ext(const Grid& g, const Cells& cells, int i, int r, double t) {
     bool neg2 = false, neg3 = false;
     if (i < 0 || i >= g.nx) {
         const int sd = i < 0 ? SIDE_XLO : SIDE_XHI;
@@ -224,15 +225,26 @@ __device__ __forceinline__ Q3 load_ext(const Grid& g, const double* __restrict__
             r = clampi(r, g.ny);
         }
     }
-    const size_t idx = (size_t)r * g.nx + i;
-    Q3 c;
-    c.q1 = q1[idx];
-    c.q2 = q2[idx];
-    c.q3 = q3[idx];
+    Q3 c = cells((size_t)r * g.nx + i);
     if (neg2) c.q2 = -c.q2;
     if (neg3) c.q3 = -c.q3;
     return c;
 }
+
+// Three planes in (global) memory, structure of arrays.
+struct PlaneCells {
+    const double *q1, *q2, *q3;
+    __device__ __forceinline__ Q3 operator()(size_t idx) const {
+        Q3 c;
+        c.q1 = q1[idx]; c.q2 = q2[idx]; c.q3 = q3[idx];
+        return c;
+    }
+};
+struct PlaneOut {
+    double *q1, *q2, *q3;
+    __device__ __forceinline__ void put(size_t idx, const Q3& c) const { q1[idx] = c.q1; q2[idx] = c.q2; q3[idx] = c.q3; }
+};
+
 
 // One-deep ghost of an intermediate state for the source step (26) (reading A9): the rule of `sd` applied to the
 // interior value `inner` (the cell next to the edge, or the wrapped one for PERIODIC -- the caller passes it).

@@ -114,9 +114,9 @@ __device__ __forceinline__ WvT<T> riemann2(const CxT<T>& L, const CxT<T>& R, T b
     const T hra = T(0.5) * ra;
     w.al1 = fma(-w.s2, D1, D2) * hra;
     w.al2 = D1 - w.al1;
-    const T wra = wv * ra;
-    w.r31 = wra * fma(T(-2), Zb2, w.s1);                         //  w (s1 - 2 Zb2)/a
-    w.r32 = wra * fma(T(2), Zb2, -w.s2);                         // -w (s2 - 2 Zb2)/a
+    const T wt = wv * ra * tt;                                   // s1 - 2 Zb2 = tt + a, s2 - 2 Zb2 = tt - a, and a/a = 1:
+    w.r31 = wv + wt;                                             //  w (s1 - 2 Zb2)/a = w + w tt/a
+    w.r32 = wv - wt;                                             // -w (s2 - 2 Zb2)/a = w - w tt/a
     w.al3 = fma(-w.al2, w.r32, fma(-w.al1, w.r31, D3));
     return w;
 }
@@ -141,9 +141,10 @@ template <class T> __device__ __forceinline__ T mc_half2(T a, T b) {
 template <class T>
 __device__ __forceinline__ FlT<T> flux2(const WvT<T>& k, T b1, T b2, T b3, T lam) {
     const T a1 = fabs(k.s1), a2 = fabs(k.s2), a3 = fabs(k.v);
-    const T f1 = a1 * fma(-lam, a1, T(1)) * mc_half2(k.al1, b1);
-    const T f2 = a2 * fma(-lam, a2, T(1)) * mc_half2(k.al2, b2);
-    const T f3 = a3 * fma(-lam, a3, T(1)) * mc_half2(k.al3, b3);
+    // |s| (1 - lam |s|) as |s| - (lam |s|) |s|: no immediate operand next to lam, which then stays in a uniform register
+    const T f1 = fma(-(lam * a1), a1, a1) * mc_half2(k.al1, b1);
+    const T f2 = fma(-(lam * a2), a2, a2) * mc_half2(k.al2, b2);
+    const T f3 = fma(-(lam * a3), a3, a3) * mc_half2(k.al3, b3);
     const T g1m = fma(Num<T>::neg_part(k.s1), k.al1, f1), g1p = fma(k.s1, k.al1, -g1m);
     const T g2m = fma(Num<T>::neg_part(k.s2), k.al2, f2), g2p = fma(k.s2, k.al2, -g2m);
     const T g3m = fma(Num<T>::neg_part(k.v), k.al3, f3), g3p = fma(k.v, k.al3, -g3m);

@@ -1,0 +1,228 @@
+// fvnl_small.cuh -- ALL time steps of a fvnl_step call in ONE launch of ONE thread-block cluster, with the state resident in
+// the cluster's DISTRIBUTED SHARED MEMORY, for grids so small that a step is bound by launches and latency, not by
+// throughput (BASELINE.json's config C1: 512 x 4 cells x 2000 steps).
+//
+// Why.  The row-marching step kernel (fvnl_ws.cuh) needs 15 ticks of ~1 us for C1's 4 rows and one launch per step:
+// ~20 us per step for 2048 cells.  Here the cells of every sub-step are spread over the threads of up to 16 CTAs on 16
+// SMs -- one thread-block cluster, the largest unit of B200 with a hardware barrier (barrier.cluster, ~0.2 us) and with
+// load/store access to each other's shared memory -- and the time loop runs INSIDE the kernel:
+//     x-sweep (24) on the y-extended mesh   -> cluster barrier
+//     y-sweep (25)                          -> cluster barrier
+//     source step (26) | a ninth warp combines the partial maxima of all CTAs and advances the CTA's copy of the
+//                        clock (the source step does not enter M)                -> cluster barrier
+// Q^n, Q* and Q** are three "distributed arrays": cell idx lives in the shared memory of CTA (idx / 256) mod C, which is
+// the CTA whose thread computes it; a neighbour's value is a plain load through the cluster's shared-memory window (~200
+// cycles remote, ~40 local; an L2 round trip is ~700 and a cluster barrier that has to publish global stores ~1.5 us:
+// the first version of this kernel, with the state in global memory, took 9.5 us per C1 step).  HBM is touched twice per
+// CALL: the state is read at the start and written at the end.  The clock (t, dt, M: PAPER.md:275-279) is kept in every
+// CTA's shared memory -- same inputs, same operations, same values -- and written back once at the end.
+// Arithmetic: the per-cell sub-step functions of the three-pass path (fvnl_unfused.cuh: every thread solves the Riemann
+// problems of its own 5-cell stencil; ghost rules and analytic source cells evaluated on load, fvnl_bc.cuh).
+#pragma once
+#include <cooperative_groups.h>
+
+#include "fvnl_fused.cuh"
+
+namespace fvnl {
+
+constexpr int SMALL_THREADS = 256;
+constexpr int SMALL_MAX_CLUSTER = 16;                      // non-portable cluster size (8 is the portable maximum)
+constexpr size_t SMALL_MAX_CELLS = 16384;                  // beyond this the row-marching kernel is faster
+
+struct SmallPartial {                                      // what one CTA contributes to the end of a step
+    unsigned long long sx, sy;                             // max |s| over its x- / y-interfaces (bit patterns)
+    int flags, pad;
+};
+
+__device__ __forceinline__ unsigned long long warp_max_bits(double v) {
+    unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long other = __shfl_xor_sync(0xffffffffu, b, o);
+        b = other > b ? other : b;
+    }
+    return b;
+}
+
+// A cell array distributed over the C = 2^logc CTAs of the cluster in blocks of SMALL_THREADS consecutive cells, round-robin:
+// three planes of `cap` doubles at the same shared-memory offset in every CTA.  Thread `tid` of CTA `rank` computes the cells
+// idx = (k C + rank) SMALL_THREADS + tid, k = 0, 1, ..., i.e. exactly the ones its own CTA stores (put is a local store).
+struct DistCells {
+    double* base;                                          // this CTA's copy of the window (generic address of shared memory)
+    int cap, logc;
+    __device__ __forceinline__ const double* where(size_t idx) const {
+        const unsigned blk = (unsigned)(idx / SMALL_THREADS), owner = blk & ((1u << logc) - 1u);
+        const double* p = base + (size_t)(blk >> logc) * SMALL_THREADS + (idx % SMALL_THREADS);
+        return cooperative_groups::this_cluster().map_shared_rank(p, owner);
+    }
+    __device__ __forceinline__ Q3 operator()(size_t idx) const {
+        const double* p = where(idx);
+        Q3 c;
+        c.q1 = p[0]; c.q2 = p[cap]; c.q3 = p[2 * cap];
+        return c;
+    }
+    __device__ __forceinline__ void put(size_t idx, const Q3& c) const {        // (idx must be one of this CTA's own)
+        double* p = base + (size_t)((unsigned)(idx / SMALL_THREADS) >> logc) * SMALL_THREADS + (idx % SMALL_THREADS);
+        p[0] = c.q1; p[cap] = c.q2; p[2 * cap] = c.q3;
+    }
+};
+
+// One cell of an x-sweep stencil, resolved ONCE before the time loop (a thread computes the same cells in every step): where
+// the ghost rules of fvnl_bc.cuh (x rule first, then y rule: load_ext) send the cell -- a pointer into the distributed Q^n,
+// the signs a REFLECT edge flips, and whether an analytic SOURCE edge may override it (that depends on t: evaluated per step).
+// Resolving it per step cost two thirds of the x-sweep's instructions (ghost-rule branches, integer divisions).
+struct StencilCell {
+    const double* p;
+    int info;                                              // bit 0: neg2, bit 1: neg3, bits 2-4: x SOURCE side + 1, bits 5-7: y SOURCE side + 1
+    short i, r, col, pad;                                  // ghost-extended position; column after the x rule
+};
+__device__ __forceinline__ StencilCell resolve_cell(const Grid& g, const DistCells& A, int i, int r) {
+    const ColMap cm = map_column(g, i);
+    const RowMap rm = map_row(g, r);
+    StencilCell e;
+    e.p = A.where((size_t)rm.row * g.nx + cm.col);
+    e.info = (cm.neg2 ? 1 : 0) | (rm.neg3 ? 2 : 0) | ((cm.xsrc + 1) << 2) | ((rm.ysrc + 1) << 5);
+    e.i = (short)i; e.r = (short)r; e.col = (short)cm.col; e.pad = 0;
+    return e;
+}
+__device__ __forceinline__ Q3 load_cell(const Grid& g, const StencilCell& e, int cap, double t) {
+    Q3 c;
+    if (e.info >> 2) {                                     // same precedence as load_ext
+        const int xs = ((e.info >> 2) & 7) - 1, ys = ((e.info >> 5) & 7) - 1;
+        if (xs >= 0 && source_at(g, xs, e.i, e.r, t, c)) return c;
+        if (ys >= 0 && source_at(g, ys, e.col, e.r, t, c)) {
+            if (e.info & 1) c.q2 = -c.q2;
+            return c;
+        }
+    }
+    c.q1 = e.p[0]; c.q2 = e.p[cap]; c.q3 = e.p[2 * cap];
+    if (e.info & 1) c.q2 = -c.q2;
+    if (e.info & 2) c.q3 = -c.q3;
+    return c;
+}
+
+// Doubles per plane and CTA for an array of n cells over C CTAs; dynamic shared memory of the kernel.
+__host__ __device__ inline int small_cap(size_t n, int C) {
+    const size_t per_round = (size_t)C * SMALL_THREADS;
+    return (int)((n + per_round - 1) / per_round) * SMALL_THREADS;
+}
+__host__ __device__ inline size_t small_smem_bytes(int nx, int ny, int C) {
+    const size_t cap = small_cap((size_t)nx * ny, C), cap_star = small_cap((size_t)nx * (ny + 4), C);
+    return 8 * 3 * (2 * cap + cap_star) + 5 * cap_star * sizeof(StencilCell);
+}
+
+// grid = cluster = C = 2^logc CTAs of SMALL_THREADS + 32 threads: SMALL_THREADS compute threads and one warp that ends the
+// step (clock) while the compute warps run the source step, which does not enter M.  Dynamic shared memory =
+// small_smem_bytes(nx, ny, C).  q1..q3: the state in global memory (in and out).  The clock must hold dt of the first step
+// (k_clock_begin) on entry.
+__global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Clock* clk, double* q1, double* q2, double* q3,
+                                                                     int logc, long long nsteps, double value, int mode) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cl = cg::this_cluster();
+    extern __shared__ __align__(16) double small_mem[];
+    const unsigned rank = cl.block_rank(), C = cl.num_blocks();
+    __shared__ SmallPartial part[2];                       // by step parity: read by the other CTAs while the next step runs
+    __shared__ Clock ck[2];                                // by step parity: the clock warp writes the next step's
+    const int tid = threadIdx.x, lane = tid & 31;
+    const bool clock_warp = tid >= SMALL_THREADS;
+    const int nx = g.nx, ny = g.ny, n = nx * ny, nstar = nx * (ny + 4);
+    const int cap = small_cap(n, C), cap_star = small_cap(nstar, C);
+    const DistCells A{small_mem, cap, logc};                                   // Q^n (and Q^{n+1})
+    const DistCells S{small_mem + 3 * cap, cap_star, logc};                    // Q* on the y-extended mesh
+    const DistCells B{small_mem + 3 * cap + 3 * cap_star, cap, logc};          // Q**
+    StencilCell* const stencil = reinterpret_cast<StencilCell*>(small_mem + 6 * cap + 3 * cap_star);   // [task k][cell e][thread]
+    const int first = (int)rank * SMALL_THREADS + tid, stride = (int)C * SMALL_THREADS;
+    const float inv_nx = 1.0f / (float)nx;                 // m / nx for m < 2^20 (exact: (m + 0.5) / nx is never near an integer)
+    if (tid == 0) { ck[0] = *clk; part[0].sx = part[0].sy = part[1].sx = part[1].sy = 0ull; part[0].flags = part[1].flags = 0; }
+    if (!clock_warp) {
+        for (int m = first; m < n; m += stride) {
+            Q3 c;
+            c.q1 = q1[m]; c.q2 = q2[m]; c.q3 = q3[m];
+            A.put(m, c);
+        }
+        for (int k = 0, m = first; m < nstar; ++k, m += stride) {
+            const int row = m / nx, i = m - row * nx;
+#pragma unroll
+            for (int e = 0; e < 5; ++e) stencil[(k * 5 + e) * SMALL_THREADS + tid] = resolve_cell(g, A, i - 2 + e, row - 2);
+        }
+    }
+    cl.sync();
+    for (long long step = 0; step < nsteps; ++step) {
+        SmallPartial* mine = &part[step & 1];
+        const Clock& now = ck[step & 1];
+        if (!clock_warp) {
+            const double t = now.t, lamx = now.lamx;
+            int flags = 0;
+            double sx = 0.0;
+            for (int k = 0, m = first; m < nstar; ++k, m += stride) {
+                Q3 v[5];
+#pragma unroll
+                for (int e = 0; e < 5; ++e) v[e] = load_cell(g, stencil[(k * 5 + e) * SMALL_THREADS + tid], cap, t);
+                const int row = __float2int_rd(((float)m + 0.5f) * inv_nx);
+                xsweep_stencil(g, lamx, v, S, m - row * nx, row - 2, sx, flags);
+            }
+            const unsigned long long bx = warp_max_bits(sx);
+            const int f = __reduce_or_sync(0xffffffffu, flags);
+            if (lane == 0) {
+                if (bx) atomicMax(&mine->sx, bx);
+                if (f) atomicOr(&mine->flags, f);
+            }
+        }
+        cl.sync();
+        if (!clock_warp) {
+            const double lamy = now.lamy;
+            int flags = 0;
+            double sy = 0.0;
+            for (int m = first; m < n; m += stride) {
+                const int row = __float2int_rd(((float)m + 0.5f) * inv_nx);
+                ysweep_cell(g, lamy, S, B, m - row * nx, row, sy, flags);
+            }
+            const unsigned long long by = warp_max_bits(sy);
+            const int f = __reduce_or_sync(0xffffffffu, flags);
+            if (lane == 0) {
+                if (by) atomicMax(&mine->sy, by);
+                if (f) atomicOr(&mine->flags, f);
+            }
+        }
+        cl.sync();
+        if (!clock_warp) {
+            const double t = now.t, kapx = now.kapx, kapy = now.kapy;
+            for (int m = first; m < n; m += stride) {
+                const int row = __float2int_rd(((float)m + 0.5f) * inv_nx);
+                source_step_cell(g, t, kapx, kapy, B, A, m - row * nx, row);
+            }
+        } else {                                           // end of the step: M_n, nu_n, t_{n+1}, dt_{n+1} (clock_advance)
+            unsigned long long bx = 0ull, by = 0ull;       // lane r fetches the partial result of CTA r
+            int f = 0;
+            if (lane < (int)C) {
+                const SmallPartial* p = cl.map_shared_rank(mine, lane);
+                bx = p->sx; by = p->sy; f = p->flags;
+            }
+            for (int o = 16; o > 0; o >>= 1) {
+                const unsigned long long ox = __shfl_xor_sync(0xffffffffu, bx, o), oy = __shfl_xor_sync(0xffffffffu, by, o);
+                bx = ox > bx ? ox : bx;
+                by = oy > by ? oy : by;
+            }
+            f = __reduce_or_sync(0xffffffffu, f);
+            if (lane == 0) {
+                Clock* next = &ck[(step + 1) & 1];
+                *next = now;
+                next->sx_bits = bx;
+                next->sy_bits = by;
+                next->flags |= f;
+                clock_advance(g, next, value, mode, step + 1 < nsteps ? 1 : 0);
+                SmallPartial* other = &part[(step + 1) & 1];               // (last read before the previous cluster barrier)
+                other->sx = other->sy = 0ull; other->flags = 0;
+            }
+        }
+        cl.sync();
+    }
+    if (!clock_warp)
+        for (int m = first; m < n; m += stride) {
+            const Q3 c = A(m);
+            q1[m] = c.q1; q2[m] = c.q2; q3[m] = c.q3;
+        }
+    if (rank == 0 && tid == 0) *clk = ck[nsteps & 1];
+    cl.sync();                                             // no CTA leaves while another may still read its shared memory
+}
+
+}  // namespace fvnl

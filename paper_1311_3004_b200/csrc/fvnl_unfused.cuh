@@ -66,49 +66,54 @@ __device__ __forceinline__ Q3 sweep_cell(const CellX c[5], double lam, double be
 }
 
 // ---- one cell of each sub-step ---------------------------------------------------------------------------------------
+// Written against "cells" (a callable idx -> Q3) and "out" (put(idx, Q3)) so that the same arithmetic serves the three-pass
+// kernels below (planes in global memory) and the small-grid cluster kernel (fvnl_small.cuh: distributed shared memory).
 // O2: Q*(i, r) of the x-sweep (24) on the y-extended mesh (row r in -2 .. ny+1 is stored at r + 2 of star).
-__device__ __forceinline__ void xsweep_cell(const Grid& g, double t, double lam, const double* q1, const double* q2,
-                                            const double* q3, double* s1, double* s2, double* s3, int i, int r, double& smax,
-                                            int& flags) {
+// v[0..4]: the cells i-2 .. i+2 of row r of the ghost-extended mesh.
+template <class Out>
+__device__ __forceinline__ void xsweep_stencil(const Grid& g, double lam, const Q3 v[5], const Out& star, int i, int r, double& smax,
+                                               int& flags) {
     CellX c[5];
     int f = 0;
 #pragma unroll
-    for (int k = 0; k < 5; ++k) {
-        const Q3 q = load_ext(g, q1, q2, q3, i - 2 + k, r, t);
-        c[k] = make_cell(q.q1, q.q2, q.q3, f);
-    }
+    for (int k = 0; k < 5; ++k) c[k] = make_cell(v[k].q1, v[k].q2, v[k].q3, f);
     double sl, sr;
     const Q3 o = sweep_cell(c, lam, 2.0 * (g.beta - 1.0), sl, sr, f);
-    const size_t idx = (size_t)(r + 2) * g.nx + i;
-    s1[idx] = o.q1; s2[idx] = o.q2; s3[idx] = o.q3;
+    star.put((size_t)(r + 2) * g.nx + i, o);
     if (r >= 0 && r < g.ny) { smax = fmax(smax, fmax(sl, sr)); flags |= f; }      // ghost rows do not enter M (O5)
+}
+template <class Cells, class Out>
+__device__ __forceinline__ void xsweep_cell(const Grid& g, double t, double lam, const Cells& q, const Out& star, int i, int r,
+                                            double& smax, int& flags) {
+    Q3 v[5];
+#pragma unroll
+    for (int k = 0; k < 5; ++k) v[k] = load_ext(g, q, i - 2 + k, r, t);
+    xsweep_stencil(g, lam, v, star, i, r, smax, flags);
 }
 
 // O3: Q**(i, j) of the y-sweep (25) of star with positions 2 and 3 switched.
-__device__ __forceinline__ void ysweep_cell(const Grid& g, double lam, const double* s1, const double* s2, const double* s3,
-                                            double* o1, double* o2, double* o3, int i, int j, double& smax, int& flags) {
+template <class Cells, class Out>
+__device__ __forceinline__ void ysweep_cell(const Grid& g, double lam, const Cells& star, const Out& out, int i, int j,
+                                            double& smax, int& flags) {
     CellX c[5];
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
-        const size_t idx = (size_t)(j + k) * g.nx + i;               // star row (j-2+k) is stored at j+k
-        c[k] = make_cell(s1[idx], s3[idx], s2[idx], flags);
+        const Q3 v = star((size_t)(j + k) * g.nx + i);               // star row (j-2+k) is stored at j+k
+        c[k] = make_cell(v.q1, v.q3, v.q2, flags);
     }
     double sl, sr;
     const Q3 o = sweep_cell(c, lam, 2.0 * (g.beta - 1.0), sl, sr, flags);
-    const size_t idx = (size_t)j * g.nx + i;
-    o1[idx] = o.q1; o2[idx] = o.q3; o3[idx] = o.q2;
+    Q3 w;
+    w.q1 = o.q1; w.q2 = o.q3; w.q3 = o.q2;
+    out.put((size_t)j * g.nx + i, w);
     smax = fmax(smax, fmax(sl, sr));
 }
 
 // O4: source step (26): q^m += kap_x d2x(q^m/q^1) + kap_y d2y(q^m/q^1), m = 2, 3 (readings A1, A2).
-__device__ __forceinline__ void source_step_cell(const Grid& g, double t, double kx, double ky, const double* a1,
-                                                 const double* a2, const double* a3, double* o1, double* o2, double* o3,
+template <class Cells, class Out>
+__device__ __forceinline__ void source_step_cell(const Grid& g, double t, double kx, double ky, const Cells& at_idx, const Out& out,
                                                  int i, int j) {
-    auto at = [&](int ii, int jj) {
-        const size_t idx = (size_t)jj * g.nx + ii;
-        Q3 c; c.q1 = a1[idx]; c.q2 = a2[idx]; c.q3 = a3[idx];
-        return c;
-    };
+    auto at = [&](int ii, int jj) { return at_idx((size_t)jj * g.nx + ii); };
     const Q3 c = at(i, j);
     Q3 w, e, s, n;
     const bool px = g.side[SIDE_XLO].kind == BC_PERIODIC, py = g.side[SIDE_YLO].kind == BC_PERIODIC;
@@ -124,10 +129,11 @@ __device__ __forceinline__ void source_step_cell(const Grid& g, double t, double
     const double z2 = c.q2 * rc, z3 = c.q3 * rc;
     const double lx2 = (e.q2 * re + w.q2 * rw) - 2.0 * z2, ly2 = (n.q2 * rn + s.q2 * rs) - 2.0 * z2;
     const double lx3 = (e.q3 * re + w.q3 * rw) - 2.0 * z3, ly3 = (n.q3 * rn + s.q3 * rs) - 2.0 * z3;
-    const size_t idx = (size_t)j * g.nx + i;
-    o1[idx] = c.q1;
-    o2[idx] = fma(ky, ly2, fma(kx, lx2, c.q2));
-    o3[idx] = fma(ky, ly3, fma(kx, lx3, c.q3));
+    Q3 o;
+    o.q1 = c.q1;
+    o.q2 = fma(ky, ly2, fma(kx, lx2, c.q2));
+    o.q3 = fma(ky, ly3, fma(kx, lx3, c.q3));
+    out.put((size_t)j * g.nx + i, o);
 }
 
 // O2 as a kernel.  grid.y = ny+4.
@@ -139,7 +145,7 @@ __global__ void __launch_bounds__(256) k_xsweep_unfused(Grid g, Clock* clk, cons
     const int r = (int)blockIdx.y - 2;
     int flags = 0;
     double smax = 0.0;
-    if (i < g.nx) xsweep_cell(g, clk->t, clk->lamx, q1, q2, q3, s1, s2, s3, i, r, smax, flags);
+    if (i < g.nx) xsweep_cell(g, clk->t, clk->lamx, PlaneCells{q1, q2, q3}, PlaneOut{s1, s2, s3}, i, r, smax, flags);
     block_max_to(&clk->sx_bits, smax);
     block_flags_to(&clk->flags, flags);
 }
@@ -151,7 +157,7 @@ __global__ void __launch_bounds__(256) k_ysweep_unfused(Grid g, Clock* clk, cons
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     int flags = 0;
     double smax = 0.0;
-    if (i < g.nx) ysweep_cell(g, clk->lamy, s1, s2, s3, o1, o2, o3, i, blockIdx.y, smax, flags);
+    if (i < g.nx) ysweep_cell(g, clk->lamy, PlaneCells{s1, s2, s3}, PlaneOut{o1, o2, o3}, i, blockIdx.y, smax, flags);
     block_max_to(&clk->sy_bits, smax);
     block_flags_to(&clk->flags, flags);
 }
@@ -161,7 +167,7 @@ __global__ void __launch_bounds__(256) k_source_unfused(Grid g, const Clock* clk
                                                         double* __restrict__ o1, double* __restrict__ o2,
                                                         double* __restrict__ o3) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < g.nx) source_step_cell(g, clk->t, clk->kapx, clk->kapy, a1, a2, a3, o1, o2, o3, i, blockIdx.y);
+    if (i < g.nx) source_step_cell(g, clk->t, clk->kapx, clk->kapy, PlaneCells{a1, a2, a3}, PlaneOut{o1, o2, o3}, i, blockIdx.y);
 }
 
 }  // namespace fvnl

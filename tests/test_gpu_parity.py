@@ -43,10 +43,11 @@ def run_both(w, steps=None, kernel=None, rows_per_block=None, chunks=None, cache
 
 
 def select(s, kernel):
-    """kernel = (FVNL_OPT_KERNEL value, FVNL_OPT_VARIANT value)."""
+    """kernel = (FVNL_OPT_KERNEL value, FVNL_OPT_VARIANT value, FVNL_OPT_SMALL_GRID value)."""
     import paper_1311_3004_b200 as P
     s.set_option(P.OPT_KERNEL, kernel[0])
     s.set_option(P.OPT_VARIANT, kernel[1])
+    s.set_option(P.OPT_SMALL_GRID, kernel[2])
 
 
 def check(w, steps=None, tol=TOL, metric=parity_error, **kw):
@@ -63,11 +64,13 @@ def check(w, steps=None, tol=TOL, metric=parity_error, **kw):
     return err
 
 
-# (FVNL_OPT_KERNEL, FVNL_OPT_VARIANT): the warp-specialised one-pass kernel k_step_ws (the default, for every kind of edge;
-# analytic SOURCE cells come from the boundary kernel / the step kernel's tail), the single-role one-pass kernel
-# k_step_fused (evaluates them in place), and the three-pass comparison kernels
-KERNELS = [(0, 0), (0, 1), (1, 0)]
-KIDS = ["ws", "fused", "unfused"]
+# (FVNL_OPT_KERNEL, FVNL_OPT_VARIANT, FVNL_OPT_SMALL_GRID): the warp-specialised one-pass kernel k_step_ws (for every kind of
+# edge; analytic SOURCE cells come from the boundary kernel / the step kernel's tail), the single-role one-pass kernel
+# k_step_fused (evaluates them in place), and the three-pass comparison kernels -- each with one launch per step -- and
+# "cluster": the library's default behaviour, in which a grid of at most 16384 cells runs all steps of a call in one launch
+# of one thread-block cluster (k_steps_cluster, fvnl_small.cuh; larger grids take the "ws" path there too)
+KERNELS = [(0, 0, 0), (0, 1, 0), (1, 0, 0), (0, 0, 1)]
+KIDS = ["ws", "fused", "unfused", "cluster"]
 
 
 @pytest.mark.parametrize("kernel", KERNELS, ids=KIDS)
