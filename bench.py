@@ -282,7 +282,9 @@ def run_gpu(args):
     spans = {names[k]: s.kernel_time(k) for k in names}
     spans = {k: v for k, v in spans.items() if v[1] > 0}
     if not per_kernel:
-        spans = {step_kernel: (ms, K)}          # one launch per step: the step IS the kernel (launch gaps included)
+        if launches < K:                        # small grid: the whole call was ONE launch of the cluster kernel (fvnl_small.cuh)
+            step_kernel = "k_steps_cluster"
+        spans = {step_kernel: (ms, K)}          # per step: the call's device time / K (launch gaps included)
     info = s.info()
 
     if rank != 0:
