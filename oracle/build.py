@@ -9,15 +9,20 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "fvnl_oracle.cpp")
-LIB = os.path.join(HERE, "libfvnl_oracle.so")
+# FVNL_ORACLE_VARIANT=fma: the SAME source compiled with FMA contraction allowed -- a second CPU program that differs from the
+# oracle by rounding only.  Used by tests/golden/make_c4_sensitivity.py alone, to measure how far two roundings of the scheme
+# drift apart on a workload; never the reference of a parity test.
+VARIANT = os.environ.get("FVNL_ORACLE_VARIANT", "")
+assert VARIANT in ("", "fma"), VARIANT
+LIB = os.path.join(HERE, "libfvnl_oracle_fma.so" if VARIANT else "libfvnl_oracle.so")
+CONTRACT = ["-ffp-contract=fast", "-mfma"] if VARIANT else ["-ffp-contract=off"]
 
 
 def build(force: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
         return LIB
     tmp = f"{LIB}.{os.getpid()}.tmp"                  # appear atomically: a running process keeps its mapped copy
-    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
-           "-shared", "-fPIC", "-o", tmp, SRC]
+    cmd = ["g++", "-std=c++17", "-O2"] + CONTRACT + ["-fno-fast-math", "-fopenmp", "-shared", "-fPIC", "-o", tmp, SRC]
     try:
         subprocess.run(cmd, check=True)
         os.replace(tmp, LIB)

@@ -329,6 +329,7 @@ extern "C" int fvnl_set_bc(fvnl_ctx* c, int side, int kind, const fvnl_source* s
     }
     c->g.side[side] = d;
     c->gvalid = false;
+    if (c->small_cluster > 0) c->small_cluster = 0;                 // (its shared-memory need depends on the SOURCE sides)
     return FVNL_OK;
 }
 
@@ -514,7 +515,7 @@ static void onepass_step(fvnl_ctx* c, double value, int mode, int more) {
 static void small_config(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* at, const fvnl_ctx* c, int cs) {
     *cfg = cudaLaunchConfig_t{};
     cfg->gridDim = dim3(cs); cfg->blockDim = dim3(SMALL_THREADS + 32); cfg->stream = c->stream;
-    cfg->dynamicSmemBytes = small_smem_bytes(c->g.nx, c->g.ny, cs);
+    cfg->dynamicSmemBytes = small_smem_bytes(c->g.nx, c->g.ny, cs, c->g.src != nullptr);
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg->attrs = at; cfg->numAttrs = 1;
@@ -526,12 +527,12 @@ static int small_cluster_size(fvnl_ctx* c) {
     if (c->small_cluster != 0) return c->small_cluster > 0 ? c->small_cluster : 0;
     c->small_cluster = -1;
     (void)cudaFuncSetAttribute(k_steps_cluster, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-    (void)cudaFuncSetAttribute(k_steps_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    (void)cudaFuncSetAttribute(k_steps_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, SMALL_MAX_SMEM);
     (void)cudaGetLastError();
     int want = 1;
     while (want < SMALL_MAX_CLUSTER && want * SMALL_THREADS < c->g.nx * (c->g.ny + 4)) want *= 2;
     for (int cs = want; cs >= 1; cs /= 2) {
-        if (small_smem_bytes(c->g.nx, c->g.ny, cs) > 200 * 1024) break;
+        if (small_smem_bytes(c->g.nx, c->g.ny, cs, c->g.src != nullptr) > (size_t)SMALL_MAX_SMEM) continue;
         cudaLaunchConfig_t cfg;
         cudaLaunchAttribute at[1];
         small_config(&cfg, at, c, cs);

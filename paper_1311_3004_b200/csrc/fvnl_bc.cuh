@@ -156,25 +156,40 @@ __device__ __forceinline__ bool source_at(const Grid& g, int sd, int i, int r, d
 }
 
 // Record n of Grid::src (layout above): the analytic cell of one ghost position at time t; q1 = -1 marks "outside the
-// aperture".  n < src_off(nx, ny, 4) / 3.
-__device__ __forceinline__ void source_record(const Grid& g, double t, size_t n, double* __restrict__ out) {
+// aperture" (and a record of a side that is not a SOURCE).  n < src_off(nx, ny, 4) / 3.
+__device__ __forceinline__ Q3 source_record_value(const Grid& g, double t, size_t n) {
+    Q3 none;
+    none.q1 = -1.0; none.q2 = 0.0; none.q3 = 0.0;
     size_t m = n;
     for (int sd = 0; sd < 4; ++sd) {
         const size_t recs = src_side_doubles(g.nx, g.ny, sd) / 3;
         if (m < recs) {
-            if (g.side[sd].kind != BC_SOURCE) return;
+            if (g.side[sd].kind != BC_SOURCE) return none;
             const int per = sd < 2 ? g.ny + 6 : g.nx;
             const int layer = (int)(m / per), pos = (int)(m % per);
             Q3 c;
             bool in;
             if (sd < 2) in = source_at(g, sd, sd == SIDE_XLO ? -1 - layer : g.nx + layer, pos - 3, t, c);
             else in = source_at(g, sd, pos, sd == SIDE_YLO ? -1 - layer : g.ny + layer, t, c);
-            double* o = out + 3 * n;
-            o[0] = in ? c.q1 : -1.0; o[1] = in ? c.q2 : 0.0; o[2] = in ? c.q3 : 0.0;
-            return;
+            return in ? c : none;
         }
         m -= recs;
     }
+    return none;
+}
+__device__ __forceinline__ void source_record(const Grid& g, double t, size_t n, double* __restrict__ out) {
+    for (int sd = 0, m = 0; sd < 4; ++sd) {                    // (records of sides that are not a SOURCE are never read)
+        m += (int)(src_side_doubles(g.nx, g.ny, sd) / 3);
+        if (n < (size_t)m) { if (g.side[sd].kind != BC_SOURCE) return; break; }
+    }
+    const Q3 c = source_record_value(g, t, n);
+    double* o = out + 3 * n;
+    o[0] = c.q1; o[1] = c.q2; o[2] = c.q3;
+}
+// Index of the record of ghost layer l (0 = next to the edge) of SOURCE side sd at position pos (row for an x side, column
+// for a y side).
+__host__ __device__ inline size_t src_record_index(int nx, int ny, int sd, int layer, int pos) {
+    return src_off(nx, ny, sd) / 3 + (sd < 2 ? (size_t)(ny + 6) * layer + (pos + 3) : (size_t)nx * layer + pos);
 }
 
 __device__ __forceinline__ int wrap(int i, int n) {

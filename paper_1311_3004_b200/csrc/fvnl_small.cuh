@@ -28,6 +28,16 @@ namespace fvnl {
 constexpr int SMALL_THREADS = 256;
 constexpr int SMALL_MAX_CLUSTER = 16;                      // non-portable cluster size (8 is the portable maximum)
 constexpr size_t SMALL_MAX_CELLS = 16384;                  // beyond this the row-marching kernel is faster
+constexpr int SMALL_MAX_SMEM = 225 * 1024;                 // dynamic shared memory a CTA may ask for (227 KB per SM, some static)
+
+// Cluster barrier between sub-steps.  Everything the sub-steps exchange lives in SHARED memory (the CTA's own or, through the
+// cluster window, another CTA's), so what has to be ordered before the arrival are this CTA's shared-memory stores: a CTA-scope
+// fence.  cooperative_groups' cluster.sync() releases at cluster scope for ALL memory, which ptxas turns into MEMBAR.ALL.GPU
+// (ncu: 8.5 % of the kernel's stall samples).
+__device__ __forceinline__ void cluster_sync_shared() {
+    __threadfence_block();
+    asm volatile("barrier.cluster.arrive.relaxed.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 
 struct SmallPartial {                                      // what one CTA contributes to the end of a step
     unsigned long long sx, sy;                             // max |s| over its x- / y-interfaces (bit patterns)
@@ -72,32 +82,55 @@ struct DistCells {
 // Resolving it per step cost two thirds of the x-sweep's instructions (ghost-rule branches, integer divisions).
 struct StencilCell {
     const double* p;
-    int info;                                              // bit 0: neg2, bit 1: neg3, bits 2-4: x SOURCE side + 1, bits 5-7: y SOURCE side + 1
-    short i, r, col, pad;                                  // ghost-extended position; column after the x rule
+    int info;                                              // bit 0: neg2, bit 1: neg3, bit 2: an analytic record may override it
+    int xrec, yrec;                                        // record of the x / y SOURCE side's analytic cell (src_record_index), -1: none
 };
 __device__ __forceinline__ StencilCell resolve_cell(const Grid& g, const DistCells& A, int i, int r) {
     const ColMap cm = map_column(g, i);
     const RowMap rm = map_row(g, r);
     StencilCell e;
     e.p = A.where((size_t)rm.row * g.nx + cm.col);
-    e.info = (cm.neg2 ? 1 : 0) | (rm.neg3 ? 2 : 0) | ((cm.xsrc + 1) << 2) | ((rm.ysrc + 1) << 5);
-    e.i = (short)i; e.r = (short)r; e.col = (short)cm.col; e.pad = 0;
+    e.xrec = e.yrec = -1;                                  // (two ghost layers: l = 0, 1)
+    if (cm.xsrc >= 0) e.xrec = (int)src_record_index(g.nx, g.ny, cm.xsrc, cm.xsrc == SIDE_XLO ? -1 - i : i - g.nx, r);
+    if (rm.ysrc >= 0) e.yrec = (int)src_record_index(g.nx, g.ny, rm.ysrc, rm.ysrc == SIDE_YLO ? -1 - r : r - g.ny, cm.col);
+    e.info = (cm.neg2 ? 1 : 0) | (rm.neg3 ? 2 : 0) | ((e.xrec >= 0 || e.yrec >= 0) ? 4 : 0);
     return e;
 }
-__device__ __forceinline__ Q3 load_cell(const Grid& g, const StencilCell& e, int cap, double t) {
-    Q3 c;
-    if (e.info >> 2) {                                     // same precedence as load_ext
-        const int xs = ((e.info >> 2) & 7) - 1, ys = ((e.info >> 5) & 7) - 1;
-        if (xs >= 0 && source_at(g, xs, e.i, e.r, t, c)) return c;
-        if (ys >= 0 && source_at(g, ys, e.col, e.r, t, c)) {
-            if (e.info & 1) c.q2 = -c.q2;
-            return c;
-        }
+// The five cells of a stencil: all fifteen loads first (no branch between them, so that they are in flight together: one
+// round trip through the cluster's shared-memory window instead of five), then the signs, then -- rare -- the analytic cells.
+// `src`: the analytic cells of this step (distributed array of records, q1 <= 0: outside the aperture / not a SOURCE side).
+__device__ __forceinline__ void load_stencil(const StencilCell* st, int stride, int cap, const DistCells& src, Q3 v[5]) {
+    int info[5], any = 0;
+#pragma unroll
+    for (int e = 0; e < 5; ++e) {
+        const StencilCell c = st[e * stride];
+        v[e].q1 = c.p[0]; v[e].q2 = c.p[cap]; v[e].q3 = c.p[2 * cap];
+        info[e] = c.info;
+        any |= c.info;
     }
-    c.q1 = e.p[0]; c.q2 = e.p[cap]; c.q3 = e.p[2 * cap];
-    if (e.info & 1) c.q2 = -c.q2;
-    if (e.info & 2) c.q3 = -c.q3;
-    return c;
+#pragma unroll
+    for (int e = 0; e < 5; ++e) {
+        v[e].q2 = (info[e] & 1) ? -v[e].q2 : v[e].q2;
+        v[e].q3 = (info[e] & 2) ? -v[e].q3 : v[e].q3;
+    }
+    if (any & 4) {                                         // a SOURCE edge in reach: same precedence as load_ext
+#pragma unroll
+        for (int e = 0; e < 5; ++e)
+            if (info[e] & 4) {
+                const StencilCell c = st[e * stride];
+                Q3 a;
+                a.q1 = -1.0;
+                if (c.xrec >= 0) a = src((size_t)c.xrec);
+                if (a.q1 > 0.0) v[e] = a;
+                else if (c.yrec >= 0) {
+                    a = src((size_t)c.yrec);
+                    if (a.q1 > 0.0) {
+                        if (c.info & 1) a.q2 = -a.q2;
+                        v[e] = a;
+                    }
+                }
+            }
+    }
 }
 
 // Doubles per plane and CTA for an array of n cells over C CTAs; dynamic shared memory of the kernel.
@@ -105,14 +138,15 @@ __host__ __device__ inline int small_cap(size_t n, int C) {
     const size_t per_round = (size_t)C * SMALL_THREADS;
     return (int)((n + per_round - 1) / per_round) * SMALL_THREADS;
 }
-__host__ __device__ inline size_t small_smem_bytes(int nx, int ny, int C) {
+__host__ __device__ inline size_t small_smem_bytes(int nx, int ny, int C, bool has_src) {
     const size_t cap = small_cap((size_t)nx * ny, C), cap_star = small_cap((size_t)nx * (ny + 4), C);
-    return 8 * 3 * (2 * cap + cap_star) + 5 * cap_star * sizeof(StencilCell);
+    const size_t cap_src = has_src ? small_cap(src_off(nx, ny, 4) / 3, C) : 0;   // analytic cells: two buffers (this / the next step)
+    return 8 * 3 * (2 * cap + cap_star + 2 * cap_src) + 5 * cap_star * sizeof(StencilCell);
 }
 
 // grid = cluster = C = 2^logc CTAs of SMALL_THREADS + 32 threads: SMALL_THREADS compute threads and one warp that ends the
 // step (clock) while the compute warps run the source step, which does not enter M.  Dynamic shared memory =
-// small_smem_bytes(nx, ny, C).  q1..q3: the state in global memory (in and out).  The clock must hold dt of the first step
+// small_smem_bytes(nx, ny, C, has_src).  q1..q3: the state in global memory (in and out).  The clock must hold dt of the first step
 // (k_clock_begin) on entry.
 __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Clock* clk, double* q1, double* q2, double* q3,
                                                                      int logc, long long nsteps, double value, int mode) {
@@ -129,11 +163,27 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
     const DistCells A{small_mem, cap, logc};                                   // Q^n (and Q^{n+1})
     const DistCells S{small_mem + 3 * cap, cap_star, logc};                    // Q* on the y-extended mesh
     const DistCells B{small_mem + 3 * cap + 3 * cap_star, cap, logc};          // Q**
-    StencilCell* const stencil = reinterpret_cast<StencilCell*>(small_mem + 6 * cap + 3 * cap_star);   // [task k][cell e][thread]
     const int first = (int)rank * SMALL_THREADS + tid, stride = (int)C * SMALL_THREADS;
+    const bool has_src = g.src != nullptr;                                     // (fvnl_step sets it when a side is a SOURCE)
+    const int nrec = (int)(src_off(nx, ny, 4) / 3), cap_src = has_src ? small_cap(nrec, C) : 0;
+    double* const src_mem = small_mem + 6 * cap + 3 * cap_star;                // analytic cells of step n: buffer n & 1
+    StencilCell* const stencil = reinterpret_cast<StencilCell*>(src_mem + 6 * cap_src);                // [task k][cell e][thread]
+    // The analytic cells of a step (two ghost layers of every SOURCE side, (41) / (43) / piston at t_n) are evaluated ONE STEP
+    // AHEAD -- t_{n+1} = t_n + dt_n is known when step n starts, PAPER.md:279 -- by the clock warp, which idles during the
+    // sweeps, each CTA the records it stores; the sweeps and the source step only load them.
+    auto make_records = [&](int buf, double t, int who, int nthreads) {
+        const DistCells R{src_mem + 3 * cap_src * buf, cap_src, logc};
+        for (int k = 0; k * stride < nrec; ++k)
+            for (int j = who; j < SMALL_THREADS; j += nthreads) {
+                const int m = k * stride + (int)rank * SMALL_THREADS + j;
+                if (m < nrec) R.put(m, source_record_value(g, t, m));
+            }
+    };
     const float inv_nx = 1.0f / (float)nx;                 // m / nx for m < 2^20 (exact: (m + 0.5) / nx is never near an integer)
     if (tid == 0) { ck[0] = *clk; part[0].sx = part[0].sy = part[1].sx = part[1].sy = 0ull; part[0].flags = part[1].flags = 0; }
+    __syncthreads();                                       // (ck[0])
     if (!clock_warp) {
+        if (has_src) make_records(0, ck[0].t, tid, SMALL_THREADS);
         for (int m = first; m < n; m += stride) {
             Q3 c;
             c.q1 = q1[m]; c.q2 = q2[m]; c.q3 = q3[m];
@@ -149,14 +199,15 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
     for (long long step = 0; step < nsteps; ++step) {
         SmallPartial* mine = &part[step & 1];
         const Clock& now = ck[step & 1];
+        const DistCells SRC{src_mem + 3 * cap_src * (int)(step & 1), cap_src, logc};
+        if (clock_warp && has_src && step + 1 < nsteps) make_records((int)((step + 1) & 1), __dadd_rn(now.t, now.dt), lane, 32);
         if (!clock_warp) {
-            const double t = now.t, lamx = now.lamx;
+            const double lamx = now.lamx;
             int flags = 0;
             double sx = 0.0;
             for (int k = 0, m = first; m < nstar; ++k, m += stride) {
                 Q3 v[5];
-#pragma unroll
-                for (int e = 0; e < 5; ++e) v[e] = load_cell(g, stencil[(k * 5 + e) * SMALL_THREADS + tid], cap, t);
+                load_stencil(stencil + (size_t)k * 5 * SMALL_THREADS + tid, SMALL_THREADS, cap, SRC, v);
                 const int row = __float2int_rd(((float)m + 0.5f) * inv_nx);
                 xsweep_stencil(g, lamx, v, S, m - row * nx, row - 2, sx, flags);
             }
@@ -167,7 +218,7 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
                 if (f) atomicOr(&mine->flags, f);
             }
         }
-        cl.sync();
+        cluster_sync_shared();
         if (!clock_warp) {
             const double lamy = now.lamy;
             int flags = 0;
@@ -183,12 +234,23 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
                 if (f) atomicOr(&mine->flags, f);
             }
         }
-        cl.sync();
+        cluster_sync_shared();
         if (!clock_warp) {
-            const double t = now.t, kapx = now.kapx, kapy = now.kapy;
+            const double kapx = now.kapx, kapy = now.kapy;
+            auto ghost = [&](int sd, const Q3& inner, int gi, int gr) {         // ghost_of, analytic cells from the records
+                const int kind = g.side[sd].kind;
+                Q3 c = inner;
+                if (kind == BC_REFLECT) {
+                    if (sd < 2) c.q2 = -c.q2; else c.q3 = -c.q3;
+                } else if (kind == BC_SOURCE) {
+                    const Q3 a = SRC(src_record_index(nx, ny, sd, 0, sd < 2 ? gr : gi));
+                    if (a.q1 > 0.0) c = a;
+                }
+                return c;
+            };
             for (int m = first; m < n; m += stride) {
                 const int row = __float2int_rd(((float)m + 0.5f) * inv_nx);
-                source_step_cell(g, t, kapx, kapy, B, A, m - row * nx, row);
+                source_step_cell(g, kapx, kapy, B, A, ghost, m - row * nx, row);
             }
         } else {                                           // end of the step: M_n, nu_n, t_{n+1}, dt_{n+1} (clock_advance)
             unsigned long long bx = 0ull, by = 0ull;       // lane r fetches the partial result of CTA r
@@ -214,7 +276,7 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
                 other->sx = other->sy = 0ull; other->flags = 0;
             }
         }
-        cl.sync();
+        cluster_sync_shared();
     }
     if (!clock_warp)
         for (int m = first; m < n; m += stride) {

@@ -110,21 +110,24 @@ __device__ __forceinline__ void ysweep_cell(const Grid& g, double lam, const Cel
 }
 
 // O4: source step (26): q^m += kap_x d2x(q^m/q^1) + kap_y d2y(q^m/q^1), m = 2, 3 (readings A1, A2).
-template <class Cells, class Out>
-__device__ __forceinline__ void source_step_cell(const Grid& g, double t, double kx, double ky, const Cells& at_idx, const Out& out,
-                                                 int i, int j) {
+// `ghost(sd, inner, i, r)`: the one-deep ghost cell of side sd at (i, r) made from the loaded cell `inner` (ghost_of).
+template <class Cells, class Out, class Ghost>
+__device__ __forceinline__ void source_step_cell(const Grid& g, double kx, double ky, const Cells& at_idx, const Out& out,
+                                                 const Ghost& ghost, int i, int j) {
     auto at = [&](int ii, int jj) { return at_idx((size_t)jj * g.nx + ii); };
-    const Q3 c = at(i, j);
-    Q3 w, e, s, n;
     const bool px = g.side[SIDE_XLO].kind == BC_PERIODIC, py = g.side[SIDE_YLO].kind == BC_PERIODIC;
-    if (i > 0) w = at(i - 1, j);
-    else w = ghost_of(g, SIDE_XLO, px ? at(g.nx - 1, j) : c, -1, j, t);
-    if (i < g.nx - 1) e = at(i + 1, j);
-    else e = ghost_of(g, SIDE_XHI, px ? at(0, j) : c, g.nx, j, t);
-    if (j > 0) s = at(i, j - 1);
-    else s = ghost_of(g, SIDE_YLO, py ? at(i, g.ny - 1) : c, i, -1, t);
-    if (j < g.ny - 1) n = at(i, j + 1);
-    else n = ghost_of(g, SIDE_YHI, py ? at(i, 0) : c, i, g.ny, t);
+    // the five loads first, independent of one another (an edge cell loads the cell its ghost is made from: the wrapped one
+    // for PERIODIC, itself otherwise), then the ghost rule on the loaded value -- rare, and the loads are all in flight by then
+    const bool xlo = i == 0, xhi = i == g.nx - 1, ylo = j == 0, yhi = j == g.ny - 1;
+    const Q3 c = at(i, j);
+    Q3 w = at(xlo ? (px ? g.nx - 1 : i) : i - 1, j);
+    Q3 e = at(xhi ? (px ? 0 : i) : i + 1, j);
+    Q3 s = at(i, ylo ? (py ? g.ny - 1 : j) : j - 1);
+    Q3 n = at(i, yhi ? (py ? 0 : j) : j + 1);
+    if (xlo) w = ghost(SIDE_XLO, w, -1, j);
+    if (xhi) e = ghost(SIDE_XHI, e, g.nx, j);
+    if (ylo) s = ghost(SIDE_YLO, s, i, -1);
+    if (yhi) n = ghost(SIDE_YHI, n, i, g.ny);
     const double rc = 1.0 / c.q1, rw = 1.0 / w.q1, re = 1.0 / e.q1, rs = 1.0 / s.q1, rn = 1.0 / n.q1;
     const double z2 = c.q2 * rc, z3 = c.q3 * rc;
     const double lx2 = (e.q2 * re + w.q2 * rw) - 2.0 * z2, ly2 = (n.q2 * rn + s.q2 * rs) - 2.0 * z2;
@@ -167,7 +170,9 @@ __global__ void __launch_bounds__(256) k_source_unfused(Grid g, const Clock* clk
                                                         double* __restrict__ o1, double* __restrict__ o2,
                                                         double* __restrict__ o3) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < g.nx) source_step_cell(g, clk->t, clk->kapx, clk->kapy, PlaneCells{a1, a2, a3}, PlaneOut{o1, o2, o3}, i, blockIdx.y);
+    const double t = clk->t;
+    auto ghost = [&](int sd, const Q3& inner, int gi, int gr) { return ghost_of(g, sd, inner, gi, gr, t); };
+    if (i < g.nx) source_step_cell(g, clk->kapx, clk->kapy, PlaneCells{a1, a2, a3}, PlaneOut{o1, o2, o3}, ghost, i, blockIdx.y);
 }
 
 }  // namespace fvnl

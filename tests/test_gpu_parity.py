@@ -458,6 +458,12 @@ def test_c4_full_size_full_step_count():
     s2.set_option(P.OPT_KERNEL, P.KERNEL_UNFUSED)
     win = gold["config"]["win"]
     done, report = 0, []
+    sens = {}                                                            # the oracle against itself under FMA contraction
+    sens_path = os.path.join(os.path.dirname(__file__), "golden", "c4_sensitivity.txt")   # (make_c4_sensitivity.py, oracle only)
+    if os.path.exists(sens_path):
+        for line in open(sens_path):
+            if line.startswith("worst"):
+                sens[int(line.split()[1])] = float(line.split()[2])
     have = [cp for cp in gold["config"]["steps"] if cp in gold["checkpoints"]]   # (a file copied from the script's .partial
     assert have and have == gold["config"]["steps"][:len(have)]                  # output holds the first checkpoints only)
     for cp in have:
@@ -487,7 +493,8 @@ def test_c4_full_size_full_step_count():
                 worst = max(worst, err)
         verdict = "within the bar" if worst <= TOL else "ABOVE THE BAR"
         print(f"PARITY C4 {w.nx}x{w.ny} step={cp} kernel=default err={worst:.3e} tol={TOL:g} {verdict}; "
-              f"default vs three-pass kernels (rounding only) drift={drift:.3e}")
+              f"default vs three-pass kernels (rounding only) drift={drift:.3e}"
+              + (f"; oracle vs oracle with FMA contraction (rounding only, same windows) {sens[cp]:.3e}" if cp in sens else ""))
         report.append((cp, worst, drift))
         if cp <= 1000:
             assert worst <= TOL, (cp, worst)

@@ -262,3 +262,29 @@ def test_c4_golden_file_is_the_full_config():
     ax = cps[3000]["windows"]["focus"]                                  # window centred on the axis: rows j0 .. j0+19
     assert ax["j0"] + 10 == w.ny // 2
     assert np.abs(ax["q"][2] + ax["q"][2][::-1]).max() <= 1e-9 * np.abs(ax["q"][2]).max()
+
+
+def test_c4_sensitivity_file_is_consistent_with_the_golden_file():
+    """tests/golden/c4_sensitivity.txt (when present): the oracle compiled with FMA contraction against the standard oracle's
+    stored C4 run -- written by tests/golden/make_c4_sensitivity.py, oracle only.  Its checkpoints are checkpoints of the
+    golden file, every window of the golden file has its three fields, 'worst' is the maximum of the step's windows, and at
+    the first checkpoint (packet still being emitted) the two roundings agree to far better than the parity bar."""
+    import os
+    mod = _load_c4_script()
+    path = os.path.join(os.path.dirname(mod.OUT), "c4_sensitivity.txt")
+    if not (os.path.exists(path) and os.path.exists(mod.OUT)):
+        pytest.skip("tests/golden/c4_sensitivity.txt not generated yet")
+    gold = mod.read()
+    windows, worst = {}, {}
+    for line in open(path):
+        if line.startswith("window"):
+            _, cp, name, m, v = line.split()
+            windows.setdefault(int(cp), {})[(name, int(m))] = float(v)
+        elif line.startswith("worst"):
+            worst[int(line.split()[1])] = float(line.split()[2])
+    assert worst and set(worst) == set(windows)
+    for cp, d in windows.items():
+        assert cp in gold["checkpoints"]
+        assert set(d) == {(name, m) for name in gold["checkpoints"][cp]["windows"] for m in range(3)}
+        assert worst[cp] == pytest.approx(max(d.values()), rel=1e-3)
+    assert worst[min(worst)] < 1e-10
