@@ -64,3 +64,17 @@ def test_product_never_touches_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in text.lower(), f"{f} mentions the oracle"
+
+
+def test_option_and_kind_constants_match_the_header():
+    """The enums of include/fvnl.h and the constants of the Python binding are the same numbers."""
+    import paper_1311_3004_b200 as P
+    src = open(os.path.join(ROOT, "include", "fvnl.h")).read()
+    found = {}
+    for body in re.findall(r"enum\s*\{(.*?)\}", src, flags=re.S):
+        for name, val in re.findall(r"(FVNL_[A-Z0-9_]+)\s*=\s*(-?\d+)", body):
+            found[name] = int(val)
+    for name in ("FVNL_OPT_KERNEL", "FVNL_OPT_ROWS_PER_BLOCK", "FVNL_OPT_KERNEL_TIMING", "FVNL_OPT_VARIANT",
+                 "FVNL_OPT_SMALL_GRID", "FVNL_KERNEL_DEFAULT", "FVNL_KERNEL_UNFUSED"):
+        assert name in found, name
+        assert getattr(P, name[len("FVNL_"):]) == found[name], name
