@@ -41,6 +41,7 @@ enum {
     FVNL_EALLOC = 2,    /* workspace too small / allocation failed                         */
     FVNL_ECUDA = 3,     /* CUDA runtime error or no device                                 */
     FVNL_ESTATE = 4,    /* call order (e.g. step before set_state)                         */
+    FVNL_ESIZE = 5,     /* grid larger than the static scratch array of fvnl_step_noalloc  */
     FVNL_ECFL = 16,     /* a step ran with nu > 1 or kappa_x + kappa_y > 1/2 */
     FVNL_ENONREAL = 32, /* square-root argument of (32),(33) negative        */
     FVNL_ENONPOS = 64,  /* q1 <= 0 met in a primitive conversion                            */
@@ -199,6 +200,31 @@ long fvnl_kernel_launches(const fvnl_ctx* ctx);
  * warps per SM, 8 chains per thread) on the current device and stream and returns the achieved rate in TFLOP/s (FMA = 2
  * flop), best of three.  Needs no context, touches no state.  Errors: FVNL_EARG, FVNL_ECUDA. */
 int fvnl_probe_fp64(void* cuda_stream, double* tflops);
+
+/* ---- ALLOCATION-FREE ENTRY POINT -------------------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ * ONE fixed-dt time step Q(t) -> Q(t + dt) of the whole path (ghost rules, x-sweep (24), y-sweep (25), source step (26);
+ * PAPER.md:147-279) by the three-pass kernels, with no context and no workspace.  The three-pass form needs scratch memory --
+ * Q* on the y-extended mesh, Q**, and the clock block (dt, lambda, kappa, running maxima, flags): here it lives in a
+ * file-scope `static __device__` array of FVNL_NOALLOC_MAX_BYTES = 16 MiB that every GPU that loads the library holds until
+ * the process exits.  The call launches five kernels on `cuda_stream` and returns without synchronising; it calls no
+ * cudaMalloc, cudaFree, cudaMemcpy or allocating library routine (the first call on a device resolves the array's device
+ * address with cudaGetSymbolAddress: make that call outside a graph capture).
+ *   q*_in / q*_out   DEVICE pointers, nx*ny doubles each (layout of fvnl_set_state), in != out; the caller owns them.
+ *   bc_kind[4]       FVNL_BC_* per side (FVNL_SIDE_* order); bc_source[s] is read for FVNL_BC_SOURCE sides only (may be NULL
+ *                    otherwise, and bc_source itself may be NULL when no side is a SOURCE).
+ *   t, dt            time at the start of the step and the time step [s] (fvnl_step's mode 0).
+ *   flags_dev        DEVICE pointer to one int that receives the step's flag word (FVNL_ECFL ... FVNL_ENAN, 0 = clean), or NULL.
+ * Limit: 6 nx ny + 12 nx + 64 doubles must fit the array (e.g. 512 x 512 or 580 x 580 cells); larger grids are rejected with
+ * FVNL_ESIZE before anything is launched.  fp64 only.
+ * Sharing: every call on a device uses the same array, which keeps the previous call's contents; the call itself resets what
+ * must start at zero (running maxima, flags).  Calls that OVERLAP on one GPU (different streams, or graphs replayed
+ * concurrently) race on it: serialise them.
+ * Errors: FVNL_EARG (as fvnl_create / fvnl_set_bc / fvnl_step, or in == out), FVNL_ESIZE, FVNL_ECUDA. */
+#define FVNL_NOALLOC_MAX_BYTES (16u << 20)
+int fvnl_step_noalloc(int nx, int ny, double dx, double dy, const fvnl_medium* medium, const int bc_kind[4],
+                      const fvnl_source* const bc_source[4], double t, double dt, const double* q1_in, const double* q2_in,
+                      const double* q3_in, double* q1_out, double* q2_out, double* q3_out, int* flags_dev, void* cuda_stream);
 
 /* Text for a status code or flag word (static storage). */
 const char* fvnl_strerror(int code);

@@ -23,7 +23,8 @@ from . import build as _build
 EXTRAP, PERIODIC, REFLECT, SOURCE = 0, 1, 2, 3
 SINE, PACKET, TANH = 0, 1, 2
 XLO, XHI, YLO, YHI = 0, 1, 2, 3
-OK, EARG, EALLOC, ECUDA, ESTATE = 0, 1, 2, 3, 4
+OK, EARG, EALLOC, ECUDA, ESTATE, ESIZE = 0, 1, 2, 3, 4, 5
+NOALLOC_MAX_BYTES = 16 << 20
 ECFL, ENONREAL, ENONPOS, ENAN = 16, 32, 64, 128
 OPT_KERNEL, OPT_ROWS_PER_BLOCK, OPT_KERNEL_TIMING, OPT_VARIANT, OPT_SMALL_GRID = 0, 1, 2, 3, 4
 TIMED_STEP, TIMED_XSWEEP, TIMED_YSWEEP, TIMED_SOURCE = 0, 1, 2, 3
@@ -74,6 +75,8 @@ def lib():
         L.fvnl_probe_fp64.argtypes = [_vp, C.POINTER(C.c_double)]
         L.fvnl_kernel_launches.restype = C.c_long
         L.fvnl_kernel_launches.argtypes = [_vp]
+        L.fvnl_step_noalloc.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(fvnl_medium), C.POINTER(C.c_int),
+                                        C.POINTER(C.POINTER(fvnl_source)), C.c_double, C.c_double] + [_vp] * 8
         L.fvnl_strerror.restype = C.c_char_p
         L.fvnl_strerror.argtypes = [C.c_int]
         _lib = L
@@ -145,6 +148,20 @@ def fvnl_probe_fp64(cuda_stream=0):
 
 def fvnl_kernel_launches(h):
     return lib().fvnl_kernel_launches(h)
+
+
+def fvnl_step_noalloc(nx, ny, dx, dy, medium, bc_kind, bc_source, t, dt, q_in, q_out, flags_ptr=0, cuda_stream=0):
+    """One fixed-dt step with no allocation (include/fvnl.h).  bc_kind: four ints; bc_source: four fvnl_source or None;
+    q_in / q_out: three DEVICE pointers (ints) each; flags_ptr: device pointer to one int, or 0."""
+    kinds = (C.c_int * 4)(*bc_kind)
+    srcs = (C.POINTER(fvnl_source) * 4)()
+    keep = []
+    for k, s in enumerate(bc_source or (None,) * 4):
+        if s is not None:
+            keep.append(s)
+            srcs[k] = C.pointer(s)
+    return lib().fvnl_step_noalloc(nx, ny, dx, dy, C.byref(medium), kinds, srcs, t, dt, *[_vp(p) for p in q_in],
+                                   *[_vp(p) for p in q_out], _vp(flags_ptr or None), _vp(cuda_stream or None))
 
 
 def fvnl_strerror(code):

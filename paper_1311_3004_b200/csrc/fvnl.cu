@@ -745,6 +745,88 @@ extern "C" int fvnl_probe_fp64(void* cuda_stream, double* tflops) {
 
 extern "C" long fvnl_kernel_launches(const fvnl_ctx* c) { return c ? c->launches : 0; }
 
+// ---------------------------------------------------------------------------------------------------------------
+// fvnl_step_noalloc: one fixed-dt step by the three-pass kernels with its scratch (clock block, Q* on the y-extended mesh,
+// Q**) in a file-scope device array -- no context, no workspace, no allocation (include/fvnl.h).  Every GPU that loads the
+// library holds the array until the process exits.  In host code `noalloc_scratch` is a host-side stand-in for the array,
+// NOT a device address: its device address is resolved once per device with cudaGetSymbolAddress and that pointer is what
+// the kernels get.
+static __device__ __align__(256) unsigned char noalloc_scratch[FVNL_NOALLOC_MAX_BYTES];
+static const int NOALLOC_CLOCK_DOUBLES = 64;                  // the clock block (sizeof(Clock) <= 512 bytes), 256-aligned
+static_assert(sizeof(Clock) <= NOALLOC_CLOCK_DOUBLES * sizeof(double), "clock block");
+static const int NOALLOC_MAX_DEVICES = 64;
+static unsigned char* noalloc_ptr[NOALLOC_MAX_DEVICES];      // device address of noalloc_scratch, per device (0: not resolved)
+
+// The clock of one stand-alone step: everything that must start at zero is cleared here (the array keeps the previous
+// call's contents), then t and the fixed dt with what derives from it.
+__global__ void k_noalloc_begin(Grid g, Clock* c, double t, double dt) {
+    c->flags = 0;
+    c->Mprev = 0.0;
+    c->last_dt = c->last_cfl = 0.0;
+    c->steps = 0;
+    c->t = t;
+    clock_set_dt(g, c, dt, 0, 0.0);                            // (also clears the running maxima and the ticket)
+}
+// End of the step: nu of the step (FVNL_ECFL if > 1) and the flag word for the caller.
+__global__ void k_noalloc_end(Grid g, Clock* c, double dt, int* flags_out) {
+    clock_advance(g, c, dt, 0, 0);
+    if (flags_out) *flags_out = c->flags;
+}
+
+extern "C" int fvnl_step_noalloc(int nx, int ny, double dx, double dy, const fvnl_medium* m, const int bc_kind[4],
+                                 const fvnl_source* const bc_source[4], double t, double dt, const double* q1_in,
+                                 const double* q2_in, const double* q3_in, double* q1_out, double* q2_out, double* q3_out,
+                                 int* flags_dev, void* cuda_stream) {
+    if (nx < 4 || ny < 4 || !(dx > 0) || !(dy > 0) || !m || !(m->c0 > 0) || !(m->rho0 > 0) || !(m->beta >= 1) ||
+        !(m->delta >= 0) || !bc_kind || !(dt > 0.0) || !(t == t))
+        return FVNL_EARG;
+    if (!q1_in || !q2_in || !q3_in || !q1_out || !q2_out || !q3_out || q1_in == q1_out || q2_in == q2_out || q3_in == q3_out)
+        return FVNL_EARG;
+    Grid g;
+    std::memset(&g, 0, sizeof(g));
+    g.nx = nx; g.ny = ny; g.dx = dx; g.dy = dy; g.c0 = m->c0; g.beta = m->beta; g.delta = m->delta;
+    for (int sd = 0; sd < 4; ++sd) {
+        const int kind = bc_kind[sd];
+        if (kind < 0 || kind > 3) return FVNL_EARG;
+        g.side[sd].kind = kind;
+        if (kind == BC_SOURCE) {
+            const fvnl_source* s = bc_source ? bc_source[sd] : nullptr;
+            if (!s || s->shape < 0 || s->shape > 2) return FVNL_EARG;
+            if (s->shape != SRC_TANH && !(s->freq_hz > 0)) return FVNL_EARG;
+            Side& d = g.side[sd];
+            d.shape = s->shape; d.amp = s->amp; d.freq_hz = s->freq_hz; d.focus_m = s->focus_m; d.centre_m = s->centre_m;
+            d.half_aperture_m = s->half_aperture_m; d.t0_s = s->t0_s; d.steep = s->steep; d.theta = s->theta;
+        }
+    }
+    for (int ax = 0; ax < 2; ++ax)
+        if ((g.side[2 * ax].kind == BC_PERIODIC) != (g.side[2 * ax + 1].kind == BC_PERIODIC)) return FVNL_EARG;
+    if (g.delta * dt / (dx * dx) + g.delta * dt / (dy * dy) > 0.5) return FVNL_EARG;
+    // ---- the scratch: [clock | Q* 3 x (ny+4) x nx | Q** 3 x ny x nx], doubles
+    const size_t n = (size_t)nx * ny, nstar = (size_t)nx * (ny + 4);
+    const size_t need = (NOALLOC_CLOCK_DOUBLES + 3 * nstar + 3 * n) * sizeof(double);
+    if (need > (size_t)FVNL_NOALLOC_MAX_BYTES) return FVNL_ESIZE;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= NOALLOC_MAX_DEVICES) { (void)cudaGetLastError(); return FVNL_ECUDA; }
+    if (!noalloc_ptr[dev]) {                                       // once per device, with that device current
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, noalloc_scratch) != cudaSuccess || !p) { (void)cudaGetLastError(); return FVNL_ECUDA; }
+        noalloc_ptr[dev] = (unsigned char*)p;
+    }
+    double* base = reinterpret_cast<double*>(noalloc_ptr[dev]);
+    Clock* clk = reinterpret_cast<Clock*>(base);
+    double* s1 = base + NOALLOC_CLOCK_DOUBLES, *s2 = s1 + nstar, *s3 = s2 + nstar;      // Q*
+    double* b1 = s3 + nstar, *b2 = b1 + n, *b3 = b2 + n;                                // Q**
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const dim3 blk(256), grd((nx + 255) / 256, ny), grdx((nx + 255) / 256, ny + 4);
+    k_noalloc_begin<<<1, 1, 0, st>>>(g, clk, t, dt);
+    k_xsweep_unfused<<<grdx, blk, 0, st>>>(g, clk, q1_in, q2_in, q3_in, s1, s2, s3);
+    k_ysweep_unfused<<<grd, blk, 0, st>>>(g, clk, s1, s2, s3, b1, b2, b3);
+    k_source_unfused<<<grd, blk, 0, st>>>(g, clk, b1, b2, b3, q1_out, q2_out, q3_out);
+    k_noalloc_end<<<1, 1, 0, st>>>(g, clk, dt, flags_dev);
+    if (cudaGetLastError() != cudaSuccess) return FVNL_ECUDA;
+    return FVNL_OK;
+}
+
 extern "C" const char* fvnl_strerror(int code) {
     switch (code) {
         case FVNL_OK: return "ok";
@@ -752,6 +834,7 @@ extern "C" const char* fvnl_strerror(int code) {
         case FVNL_EALLOC: return "workspace too small or allocation failed";
         case FVNL_ECUDA: return "CUDA error or no device";
         case FVNL_ESTATE: return "call order: no state set";
+        case FVNL_ESIZE: return "grid too large for the static scratch array of fvnl_step_noalloc (FVNL_NOALLOC_MAX_BYTES)";
         default: break;
     }
     if (code & ~(FVNL_ECFL | FVNL_ENONREAL | FVNL_ENONPOS | FVNL_ENAN)) return "unknown code";
