@@ -10,12 +10,14 @@
 //     y-sweep (25)                          -> cluster barrier
 //     source step (26) | a ninth warp combines the partial maxima of all CTAs and advances the CTA's copy of the
 //                        clock (the source step does not enter M)                -> cluster barrier
-// Q^n, Q* and Q** are three "distributed arrays": cell idx lives in the shared memory of CTA (idx / 256) mod C, which is
-// the CTA whose thread computes it; a neighbour's value is a plain load through the cluster's shared-memory window (~200
-// cycles remote, ~40 local; an L2 round trip is ~700 and a cluster barrier that has to publish global stores ~1.5 us:
-// the first version of this kernel, with the state in global memory, took 9.5 us per C1 step).  HBM is touched twice per
-// CALL: the state is read at the start and written at the end.  The clock (t, dt, M: PAPER.md:275-279) is kept in every
-// CTA's shared memory -- same inputs, same operations, same values -- and written back once at the end.
+// Q^n, Q* and Q** are three "distributed arrays": the mesh is cut into one TILE per CTA, a CTA computes and stores the cells
+// of its tile, and a neighbour's value is a plain load through the cluster's shared-memory window (~200 cycles remote, ~40
+// local; ~20 B per cycle and SM), needed for the 2-cell halo of a sweep only.  (History, C1, us per step: state in global
+// memory 9.5 -- an L2 round trip is ~700 cycles and a cluster barrier that has to publish global stores ~1.5 us; shared memory
+// with blocks of 256 consecutive cells dealt round-robin 7.6 -- every load of the x-sweep remote, half of the CTAs idle in
+// the other sub-steps; tiles 5.65.)  HBM is touched twice per CALL: the state is read at the start and written at the end.
+// The clock (t, dt, M: PAPER.md:275-279) is kept in every CTA's shared memory -- same inputs, same operations, same values --
+// and written back once at the end.
 // Arithmetic: the per-cell sub-step functions of the three-pass path (fvnl_unfused.cuh: every thread solves the Riemann
 // problems of its own 5-cell stencil; ghost rules and analytic source cells evaluated on load, fvnl_bc.cuh).
 #pragma once
@@ -53,19 +55,73 @@ __device__ __forceinline__ unsigned long long warp_max_bits(double v) {
     return b;
 }
 
-// A cell array distributed over the C = 2^logc CTAs of the cluster in blocks of SMALL_THREADS consecutive cells, round-robin:
-// three planes of `cap` doubles at the same shared-memory offset in every CTA.  Thread `tid` of CTA `rank` computes the cells
-// idx = (k C + rank) SMALL_THREADS + tid, k = 0, 1, ..., i.e. exactly the ones its own CTA stores (put is a local store).
+// How the mesh is spread over the C = Cx x Cy CTAs of the cluster: TILES of W x H cells (Q*, on the y-extended mesh of ny + 4
+// rows: W x Hs).  A CTA computes and stores the cells of its own tile, so that a sweep reads the other CTAs' shared memory
+// only for its halo (2 cells in the sweep direction), and every CTA has work in every sub-step.  (The first layout dealt
+// blocks of 256 consecutive cells round-robin: on C1 every load of the x-sweep was remote -- 30 KB per CTA and step through
+// a window that delivers ~20 B per cycle -- and half of the CTAs had no cell in the y-sweep and the source step.)
+// Cx starts at C and is halved while tiles would be narrower than 8 cells or more than twice as tall as wide.
+struct Tiling {
+    int cx_log, cy_log, W, H, Hs;
+};
+__host__ __device__ inline Tiling small_tiling(int nx, int ny, int C) {
+    int cx = C, cy = 1;
+    auto cdiv = [](int a, int b) { return (a + b - 1) / b; };
+    while (cx > 1 && (cdiv(nx, cx) < 8 || 2 * cdiv(nx, cx) < cdiv(ny, cy))) { cx /= 2; cy *= 2; }
+    Tiling t;
+    t.cx_log = 0; while ((1 << t.cx_log) < cx) ++t.cx_log;
+    t.cy_log = 0; while ((1 << t.cy_log) < cy) ++t.cy_log;
+    t.W = cdiv(nx, cx); t.H = cdiv(ny, cy); t.Hs = cdiv(ny + 4, cy);
+    return t;
+}
+// floor(a / b) for 0 <= a < 2^20, 1 <= b: (a + 0.5) / b is never within 0.5 / b of an integer, far more than fp32 rounding.
+__device__ __forceinline__ int fdiv(int a, float inv_b) { return __float2int_rd(((float)a + 0.5f) * inv_b); }
+
+// A cell array of `rows` x nx cells in tiles of W x H over the cluster: three planes of `cap` doubles at the same
+// shared-memory offset in every CTA; cell (row, col) is element (row % H) W + col % W of CTA (col / W) + Cx (row / H).
 struct DistCells {
-    double* base;                                          // this CTA's copy of the window (generic address of shared memory)
-    int cap, logc;
+    double* base;                                          // this CTA's copy (generic address of shared memory)
+    int cap, nx, W, H, cx_log;
+    float inv_nx, inv_W, inv_H;
+    __device__ __forceinline__ const double* at(int row, int col) const {
+        const int tx = fdiv(col, inv_W), ty = fdiv(row, inv_H);
+        const double* p = base + (row - ty * H) * W + (col - tx * W);
+        return cooperative_groups::this_cluster().map_shared_rank(p, (unsigned)(tx + (ty << cx_log)));
+    }
     __device__ __forceinline__ const double* where(size_t idx) const {
-        const unsigned blk = (unsigned)(idx / SMALL_THREADS), owner = blk & ((1u << logc) - 1u);
-        const double* p = base + (size_t)(blk >> logc) * SMALL_THREADS + (idx % SMALL_THREADS);
-        return cooperative_groups::this_cluster().map_shared_rank(p, owner);
+        const int row = fdiv((int)idx, inv_nx);
+        return at(row, (int)idx - row * nx);
     }
     __device__ __forceinline__ Q3 operator()(size_t idx) const {
         const double* p = where(idx);
+        Q3 c;
+        c.q1 = p[0]; c.q2 = p[cap]; c.q3 = p[2 * cap];
+        return c;
+    }
+    __device__ __forceinline__ void put(size_t idx, const Q3& c) const {        // (idx must be a cell of this CTA's tile)
+        const int row = fdiv((int)idx, inv_nx), col = (int)idx - row * nx;
+        double* p = base + (row - fdiv(row, inv_H) * H) * W + (col - fdiv(col, inv_W) * W);
+        p[0] = c.q1; p[cap] = c.q2; p[2 * cap] = c.q3;
+    }
+};
+__device__ __forceinline__ DistCells make_dist(double* base, int cap, int nx, int W, int H, int cx_log) {
+    return DistCells{base, cap, nx, W, H, cx_log, 1.0f / (float)nx, 1.0f / (float)W, 1.0f / (float)H};
+}
+// Cell number `l` (0 .. W H - 1) of the tile (tx, ty) of such an array with `rows` rows: its index row * nx + col, or -1 when it
+// lies outside the mesh (ragged last tiles).
+__device__ __forceinline__ int tile_cell(const DistCells& d, int tx, int ty, int rows, int l) {
+    const int lr = fdiv(l, d.inv_W), row = ty * d.H + lr, col = tx * d.W + (l - lr * d.W);
+    return (lr < d.H && row < rows && col < d.nx) ? row * d.nx + col : -1;
+}
+
+// The analytic records of SOURCE sides (1-D): blocks of SMALL_THREADS consecutive records dealt round-robin over the CTAs.
+struct DistRecords {
+    double* base;
+    int cap, logc;
+    __device__ __forceinline__ Q3 operator()(size_t idx) const {
+        const unsigned blk = (unsigned)(idx / SMALL_THREADS), owner = blk & ((1u << logc) - 1u);
+        const double* q = base + (size_t)(blk >> logc) * SMALL_THREADS + (idx % SMALL_THREADS);
+        const double* p = cooperative_groups::this_cluster().map_shared_rank(q, owner);
         Q3 c;
         c.q1 = p[0]; c.q2 = p[cap]; c.q3 = p[2 * cap];
         return c;
@@ -99,7 +155,7 @@ __device__ __forceinline__ StencilCell resolve_cell(const Grid& g, const DistCel
 // The five cells of a stencil: all fifteen loads first (no branch between them, so that they are in flight together: one
 // round trip through the cluster's shared-memory window instead of five), then the signs, then -- rare -- the analytic cells.
 // `src`: the analytic cells of this step (distributed array of records, q1 <= 0: outside the aperture / not a SOURCE side).
-__device__ __forceinline__ void load_stencil(const StencilCell* st, int stride, int cap, const DistCells& src, Q3 v[5]) {
+__device__ __forceinline__ void load_stencil(const StencilCell* st, int stride, int cap, const DistRecords& src, Q3 v[5]) {
     int info[5], any = 0;
 #pragma unroll
     for (int e = 0; e < 5; ++e) {
@@ -133,21 +189,23 @@ __device__ __forceinline__ void load_stencil(const StencilCell* st, int stride, 
     }
 }
 
-// Doubles per plane and CTA for an array of n cells over C CTAs; dynamic shared memory of the kernel.
-__host__ __device__ inline int small_cap(size_t n, int C) {
+// Doubles per plane and CTA; dynamic shared memory of the kernel.
+__host__ __device__ inline int small_round(int n) { return (n + SMALL_THREADS - 1) / SMALL_THREADS * SMALL_THREADS; }
+__host__ __device__ inline int small_cap_records(size_t n, int C) {
     const size_t per_round = (size_t)C * SMALL_THREADS;
     return (int)((n + per_round - 1) / per_round) * SMALL_THREADS;
 }
 __host__ __device__ inline size_t small_smem_bytes(int nx, int ny, int C, bool has_src) {
-    const size_t cap = small_cap((size_t)nx * ny, C), cap_star = small_cap((size_t)nx * (ny + 4), C);
-    const size_t cap_src = has_src ? small_cap(src_off(nx, ny, 4) / 3, C) : 0;   // analytic cells: two buffers (this / the next step)
+    const Tiling tl = small_tiling(nx, ny, C);
+    const size_t cap = small_round(tl.W * tl.H), cap_star = small_round(tl.W * tl.Hs);
+    const size_t cap_src = has_src ? small_cap_records(src_off(nx, ny, 4) / 3, C) : 0;   // two buffers (this / the next step)
     return 8 * 3 * (2 * cap + cap_star + 2 * cap_src) + 5 * cap_star * sizeof(StencilCell);
 }
 
 // grid = cluster = C = 2^logc CTAs of SMALL_THREADS + 32 threads: SMALL_THREADS compute threads and one warp that ends the
 // step (clock) while the compute warps run the source step, which does not enter M.  Dynamic shared memory =
-// small_smem_bytes(nx, ny, C, has_src).  q1..q3: the state in global memory (in and out).  The clock must hold dt of the first step
-// (k_clock_begin) on entry.
+// small_smem_bytes(nx, ny, C, has_src).  q1..q3: the state in global memory (in and out).  The clock must hold dt of the first
+// step (k_clock_begin) on entry.
 __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Clock* clk, double* q1, double* q2, double* q3,
                                                                      int logc, long long nsteps, double value, int mode) {
     namespace cg = cooperative_groups;
@@ -158,57 +216,67 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
     __shared__ Clock ck[2];                                // by step parity: the clock warp writes the next step's
     const int tid = threadIdx.x, lane = tid & 31;
     const bool clock_warp = tid >= SMALL_THREADS;
-    const int nx = g.nx, ny = g.ny, n = nx * ny, nstar = nx * (ny + 4);
-    const int cap = small_cap(n, C), cap_star = small_cap(nstar, C);
-    const DistCells A{small_mem, cap, logc};                                   // Q^n (and Q^{n+1})
-    const DistCells S{small_mem + 3 * cap, cap_star, logc};                    // Q* on the y-extended mesh
-    const DistCells B{small_mem + 3 * cap + 3 * cap_star, cap, logc};          // Q**
-    const int first = (int)rank * SMALL_THREADS + tid, stride = (int)C * SMALL_THREADS;
+    const int nx = g.nx, ny = g.ny;
+    const Tiling tl = small_tiling(nx, ny, (int)C);
+    const int tx = (int)rank & ((1 << tl.cx_log) - 1), ty = (int)rank >> tl.cx_log;      // this CTA's tile
+    const int cap = small_round(tl.W * tl.H), cap_star = small_round(tl.W * tl.Hs);
+    const int rounds = cap / SMALL_THREADS, rounds_star = cap_star / SMALL_THREADS;
+    const DistCells A = make_dist(small_mem, cap, nx, tl.W, tl.H, tl.cx_log);                              // Q^n (and Q^{n+1})
+    const DistCells S = make_dist(small_mem + 3 * cap, cap_star, nx, tl.W, tl.Hs, tl.cx_log);              // Q*, y-extended
+    const DistCells B = make_dist(small_mem + 3 * cap + 3 * cap_star, cap, nx, tl.W, tl.H, tl.cx_log);     // Q**
+    const int stride = (int)C * SMALL_THREADS;
     const bool has_src = g.src != nullptr;                                     // (fvnl_step sets it when a side is a SOURCE)
-    const int nrec = (int)(src_off(nx, ny, 4) / 3), cap_src = has_src ? small_cap(nrec, C) : 0;
+    const int nrec = (int)(src_off(nx, ny, 4) / 3), cap_src = has_src ? small_cap_records(nrec, C) : 0;
     double* const src_mem = small_mem + 6 * cap + 3 * cap_star;                // analytic cells of step n: buffer n & 1
-    StencilCell* const stencil = reinterpret_cast<StencilCell*>(src_mem + 6 * cap_src);                // [task k][cell e][thread]
+    StencilCell* const stencil = reinterpret_cast<StencilCell*>(src_mem + 6 * cap_src);                // [round k][cell e][thread]
     // The analytic cells of a step (two ghost layers of every SOURCE side, (41) / (43) / piston at t_n) are evaluated ONE STEP
     // AHEAD -- t_{n+1} = t_n + dt_n is known when step n starts, PAPER.md:279 -- by the clock warp, which idles during the
     // sweeps, each CTA the records it stores; the sweeps and the source step only load them.
     auto make_records = [&](int buf, double t, int who, int nthreads) {
-        const DistCells R{src_mem + 3 * cap_src * buf, cap_src, logc};
+        const DistRecords R{src_mem + 3 * cap_src * buf, cap_src, logc};
         for (int k = 0; k * stride < nrec; ++k)
             for (int j = who; j < SMALL_THREADS; j += nthreads) {
                 const int m = k * stride + (int)rank * SMALL_THREADS + j;
                 if (m < nrec) R.put(m, source_record_value(g, t, m));
             }
     };
-    const float inv_nx = 1.0f / (float)nx;                 // m / nx for m < 2^20 (exact: (m + 0.5) / nx is never near an integer)
     if (tid == 0) { ck[0] = *clk; part[0].sx = part[0].sy = part[1].sx = part[1].sy = 0ull; part[0].flags = part[1].flags = 0; }
     __syncthreads();                                       // (ck[0])
     if (!clock_warp) {
         if (has_src) make_records(0, ck[0].t, tid, SMALL_THREADS);
-        for (int m = first; m < n; m += stride) {
-            Q3 c;
-            c.q1 = q1[m]; c.q2 = q2[m]; c.q3 = q3[m];
-            A.put(m, c);
+        for (int k = 0; k < rounds; ++k) {
+            const int m = tile_cell(A, tx, ty, ny, k * SMALL_THREADS + tid);
+            if (m >= 0) {
+                Q3 c;
+                c.q1 = q1[m]; c.q2 = q2[m]; c.q3 = q3[m];
+                A.put(m, c);
+            }
         }
-        for (int k = 0, m = first; m < nstar; ++k, m += stride) {
-            const int row = m / nx, i = m - row * nx;
+        for (int k = 0; k < rounds_star; ++k) {
+            const int m = tile_cell(S, tx, ty, ny + 4, k * SMALL_THREADS + tid);
+            if (m >= 0) {
+                const int row = m / nx, i = m - row * nx;
 #pragma unroll
-            for (int e = 0; e < 5; ++e) stencil[(k * 5 + e) * SMALL_THREADS + tid] = resolve_cell(g, A, i - 2 + e, row - 2);
+                for (int e = 0; e < 5; ++e) stencil[(k * 5 + e) * SMALL_THREADS + tid] = resolve_cell(g, A, i - 2 + e, row - 2);
+            }
         }
     }
     cl.sync();
     for (long long step = 0; step < nsteps; ++step) {
         SmallPartial* mine = &part[step & 1];
         const Clock& now = ck[step & 1];
-        const DistCells SRC{src_mem + 3 * cap_src * (int)(step & 1), cap_src, logc};
+        const DistRecords SRC{src_mem + 3 * cap_src * (int)(step & 1), cap_src, logc};
         if (clock_warp && has_src && step + 1 < nsteps) make_records((int)((step + 1) & 1), __dadd_rn(now.t, now.dt), lane, 32);
-        if (!clock_warp) {
+        if (!clock_warp) {                                 // ---- x-sweep (24) on the y-extended mesh
             const double lamx = now.lamx;
             int flags = 0;
             double sx = 0.0;
-            for (int k = 0, m = first; m < nstar; ++k, m += stride) {
+            for (int k = 0; k < rounds_star; ++k) {
+                const int m = tile_cell(S, tx, ty, ny + 4, k * SMALL_THREADS + tid);
+                if (m < 0) continue;
                 Q3 v[5];
                 load_stencil(stencil + (size_t)k * 5 * SMALL_THREADS + tid, SMALL_THREADS, cap, SRC, v);
-                const int row = __float2int_rd(((float)m + 0.5f) * inv_nx);
+                const int row = fdiv(m, S.inv_nx);
                 xsweep_stencil(g, lamx, v, S, m - row * nx, row - 2, sx, flags);
             }
             const unsigned long long bx = warp_max_bits(sx);
@@ -219,12 +287,14 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
             }
         }
         cluster_sync_shared();
-        if (!clock_warp) {
+        if (!clock_warp) {                                 // ---- y-sweep (25)
             const double lamy = now.lamy;
             int flags = 0;
             double sy = 0.0;
-            for (int m = first; m < n; m += stride) {
-                const int row = __float2int_rd(((float)m + 0.5f) * inv_nx);
+            for (int k = 0; k < rounds; ++k) {
+                const int m = tile_cell(B, tx, ty, ny, k * SMALL_THREADS + tid);
+                if (m < 0) continue;
+                const int row = fdiv(m, B.inv_nx);
                 ysweep_cell(g, lamy, S, B, m - row * nx, row, sy, flags);
             }
             const unsigned long long by = warp_max_bits(sy);
@@ -235,7 +305,7 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
             }
         }
         cluster_sync_shared();
-        if (!clock_warp) {
+        if (!clock_warp) {                                 // ---- source step (26)
             const double kapx = now.kapx, kapy = now.kapy;
             auto ghost = [&](int sd, const Q3& inner, int gi, int gr) {         // ghost_of, analytic cells from the records
                 const int kind = g.side[sd].kind;
@@ -248,11 +318,13 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
                 }
                 return c;
             };
-            for (int m = first; m < n; m += stride) {
-                const int row = __float2int_rd(((float)m + 0.5f) * inv_nx);
+            for (int k = 0; k < rounds; ++k) {
+                const int m = tile_cell(A, tx, ty, ny, k * SMALL_THREADS + tid);
+                if (m < 0) continue;
+                const int row = fdiv(m, A.inv_nx);
                 source_step_cell(g, kapx, kapy, B, A, ghost, m - row * nx, row);
             }
-        } else {                                           // end of the step: M_n, nu_n, t_{n+1}, dt_{n+1} (clock_advance)
+        } else {                                           // ---- end of the step: M_n, nu_n, t_{n+1}, dt_{n+1} (clock_advance)
             unsigned long long bx = 0ull, by = 0ull;       // lane r fetches the partial result of CTA r
             int f = 0;
             if (lane < (int)C) {
@@ -279,9 +351,12 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
         cluster_sync_shared();
     }
     if (!clock_warp)
-        for (int m = first; m < n; m += stride) {
-            const Q3 c = A(m);
-            q1[m] = c.q1; q2[m] = c.q2; q3[m] = c.q3;
+        for (int k = 0; k < rounds; ++k) {
+            const int m = tile_cell(A, tx, ty, ny, k * SMALL_THREADS + tid);
+            if (m >= 0) {
+                const Q3 c = A(m);
+                q1[m] = c.q1; q2[m] = c.q2; q3[m] = c.q3;
+            }
         }
     if (rank == 0 && tid == 0) *clk = ck[nsteps & 1];
     cl.sync();                                             // no CTA leaves while another may still read its shared memory
