@@ -114,20 +114,20 @@ __device__ __forceinline__ int tile_cell(const DistCells& d, int tx, int ty, int
     return (lr < d.H && row < rows && col < d.nx) ? row * d.nx + col : -1;
 }
 
-// The analytic records of SOURCE sides (1-D): blocks of SMALL_THREADS consecutive records dealt round-robin over the CTAs.
+// The analytic records of SOURCE sides (1-D), dealt one by one round-robin over the CTAs: record m lives in -- and is
+// evaluated by -- CTA m mod C (in blocks of 256 the 30 records of C1's piston were all CTA 0's, whose clock warp then took
+// longer over them than the x-sweep it runs beside).
 struct DistRecords {
     double* base;
     int cap, logc;
     __device__ __forceinline__ Q3 operator()(size_t idx) const {
-        const unsigned blk = (unsigned)(idx / SMALL_THREADS), owner = blk & ((1u << logc) - 1u);
-        const double* q = base + (size_t)(blk >> logc) * SMALL_THREADS + (idx % SMALL_THREADS);
-        const double* p = cooperative_groups::this_cluster().map_shared_rank(q, owner);
+        const double* p = cooperative_groups::this_cluster().map_shared_rank(base + (idx >> logc), (unsigned)idx & ((1u << logc) - 1u));
         Q3 c;
         c.q1 = p[0]; c.q2 = p[cap]; c.q3 = p[2 * cap];
         return c;
     }
     __device__ __forceinline__ void put(size_t idx, const Q3& c) const {        // (idx must be one of this CTA's own)
-        double* p = base + (size_t)((unsigned)(idx / SMALL_THREADS) >> logc) * SMALL_THREADS + (idx % SMALL_THREADS);
+        double* p = base + (idx >> logc);
         p[0] = c.q1; p[cap] = c.q2; p[2 * cap] = c.q3;
     }
 };
@@ -170,31 +170,82 @@ __device__ __forceinline__ void load_stencil(const StencilCell* st, int stride, 
         v[e].q3 = (info[e] & 2) ? -v[e].q3 : v[e].q3;
     }
     if (any & 4) {                                         // a SOURCE edge in reach: same precedence as load_ext
+        Q3 ax[5], ay[5];                                   // both candidate records of every such cell first: the loads (remote,
+#pragma unroll                                             // ~250 cycles each) are then in flight together
+        for (int e = 0; e < 5; ++e) {
+            ax[e].q1 = ay[e].q1 = -1.0;
+            if (info[e] & 4) {
+                const StencilCell c = st[e * stride];
+                if (c.xrec >= 0) ax[e] = src((size_t)c.xrec);
+                if (c.yrec >= 0) ay[e] = src((size_t)c.yrec);
+            }
+        }
 #pragma unroll
         for (int e = 0; e < 5; ++e)
             if (info[e] & 4) {
-                const StencilCell c = st[e * stride];
-                Q3 a;
-                a.q1 = -1.0;
-                if (c.xrec >= 0) a = src((size_t)c.xrec);
-                if (a.q1 > 0.0) v[e] = a;
-                else if (c.yrec >= 0) {
-                    a = src((size_t)c.yrec);
-                    if (a.q1 > 0.0) {
-                        if (c.info & 1) a.q2 = -a.q2;
-                        v[e] = a;
-                    }
+                if (ax[e].q1 > 0.0) v[e] = ax[e];
+                else if (ay[e].q1 > 0.0) {
+                    if (info[e] & 1) ay[e].q2 = -ay[e].q2;
+                    v[e] = ay[e];
                 }
             }
     }
 }
 
+// max over the warp of non-negative doubles given as bit patterns: two 32-bit REDUX instead of five shuffle rounds.
+__device__ __forceinline__ unsigned long long warp_max_bits_redux(unsigned long long b) {
+    const unsigned hi = (unsigned)(b >> 32), lo = (unsigned)b;
+    const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
+    const unsigned ml = __reduce_max_sync(0xffffffffu, hi == mh ? lo : 0u);
+    return ((unsigned long long)mh << 32) | ml;
+}
+
+// clock_advance (fvnl_bc.cuh) by a whole warp: the same operations on the same operands -- bitwise the same clock -- but the
+// IEEE divisions that do not depend on one another run in different lanes (sx/dx and sy/dy; then lambda_x, lambda_y, kappa_x,
+// kappa_y), so that the chain is three divisions long instead of seven.  sx_bits / sy_bits / flags: the step's maxima and
+// flag word, the same in every lane.  Lane 0 writes *next.  All 32 lanes must call it.
+__device__ __forceinline__ void clock_advance_warp(const Grid& g, const Clock& now, Clock* next, unsigned long long sx_bits,
+                                                   unsigned long long sy_bits, int flags, double value, int mode, int more, int lane) {
+    const double s = __longlong_as_double((long long)((lane & 1) ? sy_bits : sx_bits));
+    const double q = __ddiv_rn(s, (lane & 1) ? g.dy : g.dx);
+    const double M = fmax(__shfl_sync(0xffffffffu, q, 0), __shfl_sync(0xffffffffu, q, 1));
+    const double dt_old = now.dt;
+    const double cfl = __dmul_rn(__dmul_rn(g.c0, dt_old), M);
+    int fl = now.flags | flags;
+    if (cfl > 1.0) fl |= F_ECFL;
+    double dt = dt_old, r = 0.0;
+    if (more) {                                            // clock_set_dt
+        dt = (mode == 1) ? __ddiv_rn(value, __dmul_rn(g.c0, M)) : value;
+        const double num = __dmul_rn(lane < 2 ? g.c0 : g.delta, dt);
+        const double den = lane == 0 ? g.dx : lane == 1 ? g.dy : lane == 2 ? __dmul_rn(g.dx, g.dx) : __dmul_rn(g.dy, g.dy);
+        r = __ddiv_rn(num, den);
+    }
+    const double lamx = __shfl_sync(0xffffffffu, r, 0), lamy = __shfl_sync(0xffffffffu, r, 1),
+                 kapx = __shfl_sync(0xffffffffu, r, 2), kapy = __shfl_sync(0xffffffffu, r, 3);
+    if (lane == 0) {
+        *next = now;
+        next->last_dt = dt_old;
+        next->last_cfl = cfl;
+        next->Mprev = M;
+        next->t = __dadd_rn(now.t, dt_old);
+        next->steps = now.steps + 1;
+        next->ticket = 0u;
+        next->sx_bits = sx_bits;                           // (as clock_advance leaves them when no step follows)
+        next->sy_bits = sy_bits;
+        if (more) {
+            next->dt = dt; next->lamx = lamx; next->lamy = lamy; next->kapx = kapx; next->kapy = kapy;
+            if (__dadd_rn(kapx, kapy) > 0.5) fl |= F_ECFL;
+            if (!(dt > 0.0) || not_finite(dt)) fl |= F_ENAN;
+            next->sx_bits = 0ull;
+            next->sy_bits = 0ull;
+        }
+        next->flags = fl;
+    }
+}
+
 // Doubles per plane and CTA; dynamic shared memory of the kernel.
 __host__ __device__ inline int small_round(int n) { return (n + SMALL_THREADS - 1) / SMALL_THREADS * SMALL_THREADS; }
-__host__ __device__ inline int small_cap_records(size_t n, int C) {
-    const size_t per_round = (size_t)C * SMALL_THREADS;
-    return (int)((n + per_round - 1) / per_round) * SMALL_THREADS;
-}
+__host__ __device__ inline int small_cap_records(size_t n, int C) { return (int)((n + C - 1) / C + 1) & ~1; }
 __host__ __device__ inline size_t small_smem_bytes(int nx, int ny, int C, bool has_src) {
     const Tiling tl = small_tiling(nx, ny, C);
     const size_t cap = small_round(tl.W * tl.H), cap_star = small_round(tl.W * tl.Hs);
@@ -224,7 +275,6 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
     const DistCells A = make_dist(small_mem, cap, nx, tl.W, tl.H, tl.cx_log);                              // Q^n (and Q^{n+1})
     const DistCells S = make_dist(small_mem + 3 * cap, cap_star, nx, tl.W, tl.Hs, tl.cx_log);              // Q*, y-extended
     const DistCells B = make_dist(small_mem + 3 * cap + 3 * cap_star, cap, nx, tl.W, tl.H, tl.cx_log);     // Q**
-    const int stride = (int)C * SMALL_THREADS;
     const bool has_src = g.src != nullptr;                                     // (fvnl_step sets it when a side is a SOURCE)
     const int nrec = (int)(src_off(nx, ny, 4) / 3), cap_src = has_src ? small_cap_records(nrec, C) : 0;
     double* const src_mem = small_mem + 6 * cap + 3 * cap_star;                // analytic cells of step n: buffer n & 1
@@ -234,11 +284,20 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
     // sweeps, each CTA the records it stores; the sweeps and the source step only load them.
     auto make_records = [&](int buf, double t, int who, int nthreads) {
         const DistRecords R{src_mem + 3 * cap_src * buf, cap_src, logc};
-        for (int k = 0; k * stride < nrec; ++k)
-            for (int j = who; j < SMALL_THREADS; j += nthreads) {
-                const int m = k * stride + (int)rank * SMALL_THREADS + j;
-                if (m < nrec) R.put(m, source_record_value(g, t, m));
+        for (int sd = 0; sd < 4; ++sd) {                   // only the records of SOURCE sides exist for the readers
+            if (g.side[sd].kind != BC_SOURCE) continue;
+            const int first = (int)(src_off(nx, ny, sd) / 3), cnt = (int)(src_side_doubles(nx, ny, sd) / 3);
+            const int per = sd < 2 ? ny + 6 : nx;          // records per ghost layer (layout of Grid::src, fvnl_bc.cuh)
+            for (int m = first + (((int)rank - first) & ((int)C - 1)) + (int)C * who; m < first + cnt; m += (int)C * nthreads) {
+                const int layer = (m - first) / per, pos = (m - first) - layer * per;
+                Q3 c;
+                bool in;
+                if (sd < 2) in = source_at(g, sd, sd == SIDE_XLO ? -1 - layer : nx + layer, pos - 3, t, c);
+                else in = source_at(g, sd, pos, sd == SIDE_YLO ? -1 - layer : ny + layer, t, c);
+                if (!in) { c.q1 = -1.0; c.q2 = c.q3 = 0.0; }
+                R.put(m, c);
             }
+        }
     };
     if (tid == 0) { ck[0] = *clk; part[0].sx = part[0].sy = part[1].sx = part[1].sy = 0ull; part[0].flags = part[1].flags = 0; }
     __syncthreads();                                       // (ck[0])
@@ -331,19 +390,11 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
                 const SmallPartial* p = cl.map_shared_rank(mine, lane);
                 bx = p->sx; by = p->sy; f = p->flags;
             }
-            for (int o = 16; o > 0; o >>= 1) {
-                const unsigned long long ox = __shfl_xor_sync(0xffffffffu, bx, o), oy = __shfl_xor_sync(0xffffffffu, by, o);
-                bx = ox > bx ? ox : bx;
-                by = oy > by ? oy : by;
-            }
+            bx = warp_max_bits_redux(bx);
+            by = warp_max_bits_redux(by);
             f = __reduce_or_sync(0xffffffffu, f);
+            clock_advance_warp(g, now, &ck[(step + 1) & 1], bx, by, f, value, mode, step + 1 < nsteps ? 1 : 0, lane);
             if (lane == 0) {
-                Clock* next = &ck[(step + 1) & 1];
-                *next = now;
-                next->sx_bits = bx;
-                next->sy_bits = by;
-                next->flags |= f;
-                clock_advance(g, next, value, mode, step + 1 < nsteps ? 1 : 0);
                 SmallPartial* other = &part[(step + 1) & 1];               // (last read before the previous cluster barrier)
                 other->sx = other->sy = 0ull; other->flags = 0;
             }
