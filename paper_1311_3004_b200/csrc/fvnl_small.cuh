@@ -92,6 +92,17 @@ struct DistCells {
         const int row = fdiv((int)idx, inv_nx);
         return at(row, (int)idx - row * nx);
     }
+    // cell (row, col) as a 32-bit code, owner << 24 | offset in the owner's plane, and the cell behind such a code
+    __device__ __forceinline__ unsigned code(int row, int col) const {
+        const int tx = fdiv(col, inv_W), ty = fdiv(row, inv_H);
+        return (unsigned)((tx + (ty << cx_log)) << 24) | (unsigned)((row - ty * H) * W + (col - tx * W));
+    }
+    __device__ __forceinline__ Q3 by_code(unsigned code) const {
+        const double* p = cooperative_groups::this_cluster().map_shared_rank(base + (code & 0xffffffu), code >> 24);
+        Q3 c;
+        c.q1 = p[0]; c.q2 = p[cap]; c.q3 = p[2 * cap];
+        return c;
+    }
     __device__ __forceinline__ Q3 operator()(size_t idx) const {
         const double* p = where(idx);
         Q3 c;
@@ -170,23 +181,20 @@ __device__ __forceinline__ void load_stencil(const StencilCell* st, int stride, 
         v[e].q3 = (info[e] & 2) ? -v[e].q3 : v[e].q3;
     }
     if (any & 4) {                                         // a SOURCE edge in reach: same precedence as load_ext
-        Q3 ax[5], ay[5];                                   // both candidate records of every such cell first: the loads (remote,
-#pragma unroll                                             // ~250 cycles each) are then in flight together
-        for (int e = 0; e < 5; ++e) {
-            ax[e].q1 = ay[e].q1 = -1.0;
-            if (info[e] & 4) {
-                const StencilCell c = st[e * stride];
-                if (c.xrec >= 0) ax[e] = src((size_t)c.xrec);
-                if (c.yrec >= 0) ay[e] = src((size_t)c.yrec);
-            }
-        }
 #pragma unroll
         for (int e = 0; e < 5; ++e)
             if (info[e] & 4) {
-                if (ax[e].q1 > 0.0) v[e] = ax[e];
-                else if (ay[e].q1 > 0.0) {
-                    if (info[e] & 1) ay[e].q2 = -ay[e].q2;
-                    v[e] = ay[e];
+                const StencilCell c = st[e * stride];
+                Q3 a;
+                a.q1 = -1.0;
+                if (c.xrec >= 0) a = src((size_t)c.xrec);
+                if (a.q1 > 0.0) v[e] = a;
+                else if (c.yrec >= 0) {
+                    a = src((size_t)c.yrec);
+                    if (a.q1 > 0.0) {
+                        if (c.info & 1) a.q2 = -a.q2;
+                        v[e] = a;
+                    }
                 }
             }
     }
@@ -243,6 +251,17 @@ __device__ __forceinline__ void clock_advance_warp(const Grid& g, const Clock& n
     }
 }
 
+// One cell of the source step, resolved once before the time loop (as StencilCell for the x-sweep): where its four neighbours
+// live in Q** (for an edge cell: the cell its ghost is made from -- the wrapped one for PERIODIC, itself otherwise), its own
+// offset in the CTA's planes of Q** and Q^n, its position and which edges it touches.
+struct SrcCell {
+    unsigned w, e, s, n;                                   // DistCells::code
+    int own;                                               // offset in this CTA's plane; -1: no cell
+    short i, j;
+    int edge;                                              // bit 0: x-lo, 1: x-hi, 2: y-lo, 3: y-hi
+    int pad;
+};
+
 // Doubles per plane and CTA; dynamic shared memory of the kernel.
 __host__ __device__ inline int small_round(int n) { return (n + SMALL_THREADS - 1) / SMALL_THREADS * SMALL_THREADS; }
 __host__ __device__ inline int small_cap_records(size_t n, int C) { return (int)((n + C - 1) / C + 1) & ~1; }
@@ -250,7 +269,7 @@ __host__ __device__ inline size_t small_smem_bytes(int nx, int ny, int C, bool h
     const Tiling tl = small_tiling(nx, ny, C);
     const size_t cap = small_round(tl.W * tl.H), cap_star = small_round(tl.W * tl.Hs);
     const size_t cap_src = has_src ? small_cap_records(src_off(nx, ny, 4) / 3, C) : 0;   // two buffers (this / the next step)
-    return 8 * 3 * (2 * cap + cap_star + 2 * cap_src) + 5 * cap_star * sizeof(StencilCell);
+    return 8 * 3 * (2 * cap + cap_star + 2 * cap_src) + 5 * cap_star * sizeof(StencilCell) + cap * sizeof(SrcCell);
 }
 
 // grid = cluster = C = 2^logc CTAs of SMALL_THREADS + 32 threads: SMALL_THREADS compute threads and one warp that ends the
@@ -279,6 +298,7 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
     const int nrec = (int)(src_off(nx, ny, 4) / 3), cap_src = has_src ? small_cap_records(nrec, C) : 0;
     double* const src_mem = small_mem + 6 * cap + 3 * cap_star;                // analytic cells of step n: buffer n & 1
     StencilCell* const stencil = reinterpret_cast<StencilCell*>(src_mem + 6 * cap_src);                // [round k][cell e][thread]
+    SrcCell* const stab = reinterpret_cast<SrcCell*>(stencil + 5 * cap_star);                          // [round k][thread]
     // The analytic cells of a step (two ghost layers of every SOURCE side, (41) / (43) / piston at t_n) are evaluated ONE STEP
     // AHEAD -- t_{n+1} = t_n + dt_n is known when step n starts, PAPER.md:279 -- by the clock warp, which idles during the
     // sweeps, each CTA the records it stores; the sweeps and the source step only load them.
@@ -310,6 +330,24 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
                 c.q1 = q1[m]; c.q2 = q2[m]; c.q3 = q3[m];
                 A.put(m, c);
             }
+        }
+        const bool px = g.side[SIDE_XLO].kind == BC_PERIODIC, py = g.side[SIDE_YLO].kind == BC_PERIODIC;
+        for (int k = 0; k < rounds; ++k) {                 // the source step's cells (same choices as source_step_cell)
+            const int m = tile_cell(A, tx, ty, ny, k * SMALL_THREADS + tid);
+            SrcCell c;
+            c.own = -1; c.w = c.e = c.s = c.n = 0u; c.i = c.j = 0; c.edge = 0; c.pad = 0;
+            if (m >= 0) {
+                const int j = m / nx, i = m - j * nx;
+                const bool xlo = i == 0, xhi = i == nx - 1, ylo = j == 0, yhi = j == ny - 1;
+                c.own = (int)(B.code(j, i) & 0xffffffu);
+                c.w = B.code(j, xlo ? (px ? nx - 1 : i) : i - 1);
+                c.e = B.code(j, xhi ? (px ? 0 : i) : i + 1);
+                c.s = B.code(ylo ? (py ? ny - 1 : j) : j - 1, i);
+                c.n = B.code(yhi ? (py ? 0 : j) : j + 1, i);
+                c.i = (short)i; c.j = (short)j;
+                c.edge = (xlo ? 1 : 0) | (xhi ? 2 : 0) | (ylo ? 4 : 0) | (yhi ? 8 : 0);
+            }
+            stab[k * SMALL_THREADS + tid] = c;
         }
         for (int k = 0; k < rounds_star; ++k) {
             const int m = tile_cell(S, tx, ty, ny + 4, k * SMALL_THREADS + tid);
@@ -378,10 +416,21 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
                 return c;
             };
             for (int k = 0; k < rounds; ++k) {
-                const int m = tile_cell(A, tx, ty, ny, k * SMALL_THREADS + tid);
-                if (m < 0) continue;
-                const int row = fdiv(m, A.inv_nx);
-                source_step_cell(g, kapx, kapy, B, A, ghost, m - row * nx, row);
+                const SrcCell sc = stab[k * SMALL_THREADS + tid];
+                if (sc.own < 0) continue;
+                const double* pc = B.base + sc.own;        // five independent loads, then -- rare -- the ghost rules
+                Q3 c;
+                c.q1 = pc[0]; c.q2 = pc[cap]; c.q3 = pc[2 * cap];
+                Q3 w = B.by_code(sc.w), e = B.by_code(sc.e), s = B.by_code(sc.s), n = B.by_code(sc.n);
+                if (sc.edge) {
+                    if (sc.edge & 1) w = ghost(SIDE_XLO, w, -1, sc.j);
+                    if (sc.edge & 2) e = ghost(SIDE_XHI, e, nx, sc.j);
+                    if (sc.edge & 4) s = ghost(SIDE_YLO, s, sc.i, -1);
+                    if (sc.edge & 8) n = ghost(SIDE_YHI, n, sc.i, ny);
+                }
+                const Q3 o = source_step_values(c, w, e, s, n, kapx, kapy);
+                double* pa = A.base + sc.own;
+                pa[0] = o.q1; pa[cap] = o.q2; pa[2 * cap] = o.q3;
             }
         } else {                                           // ---- end of the step: M_n, nu_n, t_{n+1}, dt_{n+1} (clock_advance)
             unsigned long long bx = 0ull, by = 0ull;       // lane r fetches the partial result of CTA r

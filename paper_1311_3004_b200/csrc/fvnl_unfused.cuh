@@ -109,7 +109,19 @@ __device__ __forceinline__ void ysweep_cell(const Grid& g, double lam, const Cel
     smax = fmax(smax, fmax(sl, sr));
 }
 
-// O4: source step (26): q^m += kap_x d2x(q^m/q^1) + kap_y d2y(q^m/q^1), m = 2, 3 (readings A1, A2).
+// O4: source step (26): q^m += kap_x d2x(q^m/q^1) + kap_y d2y(q^m/q^1), m = 2, 3 (readings A1, A2), from
+// the cell and its four neighbours (ghost rule already applied).
+__device__ __forceinline__ Q3 source_step_values(const Q3& c, const Q3& w, const Q3& e, const Q3& s, const Q3& n, double kx, double ky) {
+    const double rc = 1.0 / c.q1, rw = 1.0 / w.q1, re = 1.0 / e.q1, rs = 1.0 / s.q1, rn = 1.0 / n.q1;
+    const double z2 = c.q2 * rc, z3 = c.q3 * rc;
+    const double lx2 = (e.q2 * re + w.q2 * rw) - 2.0 * z2, ly2 = (n.q2 * rn + s.q2 * rs) - 2.0 * z2;
+    const double lx3 = (e.q3 * re + w.q3 * rw) - 2.0 * z3, ly3 = (n.q3 * rn + s.q3 * rs) - 2.0 * z3;
+    Q3 o;
+    o.q1 = c.q1;
+    o.q2 = fma(ky, ly2, fma(kx, lx2, c.q2));
+    o.q3 = fma(ky, ly3, fma(kx, lx3, c.q3));
+    return o;
+}
 // `ghost(sd, inner, i, r)`: the one-deep ghost cell of side sd at (i, r) made from the loaded cell `inner` (ghost_of).
 template <class Cells, class Out, class Ghost>
 __device__ __forceinline__ void source_step_cell(const Grid& g, double kx, double ky, const Cells& at_idx, const Out& out,
@@ -128,15 +140,7 @@ __device__ __forceinline__ void source_step_cell(const Grid& g, double kx, doubl
     if (xhi) e = ghost(SIDE_XHI, e, g.nx, j);
     if (ylo) s = ghost(SIDE_YLO, s, i, -1);
     if (yhi) n = ghost(SIDE_YHI, n, i, g.ny);
-    const double rc = 1.0 / c.q1, rw = 1.0 / w.q1, re = 1.0 / e.q1, rs = 1.0 / s.q1, rn = 1.0 / n.q1;
-    const double z2 = c.q2 * rc, z3 = c.q3 * rc;
-    const double lx2 = (e.q2 * re + w.q2 * rw) - 2.0 * z2, ly2 = (n.q2 * rn + s.q2 * rs) - 2.0 * z2;
-    const double lx3 = (e.q3 * re + w.q3 * rw) - 2.0 * z3, ly3 = (n.q3 * rn + s.q3 * rs) - 2.0 * z3;
-    Q3 o;
-    o.q1 = c.q1;
-    o.q2 = fma(ky, ly2, fma(kx, lx2, c.q2));
-    o.q3 = fma(ky, ly3, fma(kx, lx3, c.q3));
-    out.put((size_t)j * g.nx + i, o);
+    out.put((size_t)j * g.nx + i, source_step_values(c, w, e, s, n, kx, ky));
 }
 
 // O2 as a kernel.  grid.y = ny+4.
