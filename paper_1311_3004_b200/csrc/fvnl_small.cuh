@@ -150,7 +150,7 @@ struct DistRecords {
 struct StencilCell {
     const double* p;
     int info;                                              // bit 0: neg2, bit 1: neg3, bit 2: an analytic record may override it
-    int xrec, yrec;                                        // record of the x / y SOURCE side's analytic cell (src_record_index), -1: none
+    int xrec, yrec;                                        // analytic cell of the x / y SOURCE side: local slot / record (src_record_index), -1: none
 };
 __device__ __forceinline__ StencilCell resolve_cell(const Grid& g, const DistCells& A, int i, int r) {
     const ColMap cm = map_column(g, i);
@@ -166,7 +166,10 @@ __device__ __forceinline__ StencilCell resolve_cell(const Grid& g, const DistCel
 // The five cells of a stencil: all fifteen loads first (no branch between them, so that they are in flight together: one
 // round trip through the cluster's shared-memory window instead of five), then the signs, then -- rare -- the analytic cells.
 // `src`: the analytic cells of this step (distributed array of records, q1 <= 0: outside the aperture / not a SOURCE side).
-__device__ __forceinline__ void load_stencil(const StencilCell* st, int stride, int cap, const DistRecords& src, Q3 v[5]) {
+// `src`: the analytic cells of y sides of this step (distributed records); `xs`, `ns`: those of x sides this CTA's threads read,
+// in its own shared memory (three planes of ns doubles; StencilCell::xrec is the slot).
+__device__ __forceinline__ void load_stencil(const StencilCell* st, int stride, int cap, const DistRecords& src, const double* xs, int ns,
+                                             Q3 v[5]) {
     int info[5], any = 0;
 #pragma unroll
     for (int e = 0; e < 5; ++e) {
@@ -187,7 +190,7 @@ __device__ __forceinline__ void load_stencil(const StencilCell* st, int stride, 
                 const StencilCell c = st[e * stride];
                 Q3 a;
                 a.q1 = -1.0;
-                if (c.xrec >= 0) a = src((size_t)c.xrec);
+                if (c.xrec >= 0) { a.q1 = xs[c.xrec]; a.q2 = xs[ns + c.xrec]; a.q3 = xs[2 * ns + c.xrec]; }
                 if (a.q1 > 0.0) v[e] = a;
                 else if (c.yrec >= 0) {
                     a = src((size_t)c.yrec);
@@ -259,9 +262,12 @@ struct SrcCell {
     int own;                                               // offset in this CTA's plane; -1: no cell
     short i, j;
     int edge;                                              // bit 0: x-lo, 1: x-hi, 2: y-lo, 3: y-hi
-    int pad;
+    int xslot;                                             // local slot of the x side's analytic ghost cell, -1: none
 };
 
+// Local slots for the analytic cells of x sides a CTA's threads read: per row of its Q* tile at most three ghost cells on each
+// side (columns -2, -1 from column 0's stencil, -1 from column 1's; duplicates get slots of their own), plus the source step's.
+__host__ __device__ inline int small_xslots(const Tiling& tl) { return (6 * tl.Hs + 2 * tl.H + 3) & ~3; }
 // Doubles per plane and CTA; dynamic shared memory of the kernel.
 __host__ __device__ inline int small_round(int n) { return (n + SMALL_THREADS - 1) / SMALL_THREADS * SMALL_THREADS; }
 __host__ __device__ inline int small_cap_records(size_t n, int C) { return (int)((n + C - 1) / C + 1) & ~1; }
@@ -269,7 +275,8 @@ __host__ __device__ inline size_t small_smem_bytes(int nx, int ny, int C, bool h
     const Tiling tl = small_tiling(nx, ny, C);
     const size_t cap = small_round(tl.W * tl.H), cap_star = small_round(tl.W * tl.Hs);
     const size_t cap_src = has_src ? small_cap_records(src_off(nx, ny, 4) / 3, C) : 0;   // two buffers (this / the next step)
-    return 8 * 3 * (2 * cap + cap_star + 2 * cap_src) + 5 * cap_star * sizeof(StencilCell) + cap * sizeof(SrcCell);
+    const size_t ns = has_src ? small_xslots(tl) : 0;
+    return 8 * 3 * (2 * cap + cap_star + 2 * cap_src + 2 * ns) + 5 * cap_star * sizeof(StencilCell) + cap * sizeof(SrcCell) + 4 * ns;
 }
 
 // grid = cluster = C = 2^logc CTAs of SMALL_THREADS + 32 threads: SMALL_THREADS compute threads and one warp that ends the
@@ -299,12 +306,22 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
     double* const src_mem = small_mem + 6 * cap + 3 * cap_star;                // analytic cells of step n: buffer n & 1
     StencilCell* const stencil = reinterpret_cast<StencilCell*>(src_mem + 6 * cap_src);                // [round k][cell e][thread]
     SrcCell* const stab = reinterpret_cast<SrcCell*>(stencil + 5 * cap_star);                          // [round k][thread]
+    const int ns = has_src ? small_xslots(tl) : 0;         // local slots: the analytic cells of x sides this CTA's threads read
+    double* const xs_mem = reinterpret_cast<double*>(stab + cap);                                      // [buffer][3][ns]
+    int* const slot_rec = reinterpret_cast<int*>(xs_mem + 6 * ns);                                     // record of a slot
+    __shared__ int nslots;
+    auto new_slot = [&](int rec) {                         // (set-up only)
+        const int sl = atomicAdd(&nslots, 1);
+        if (sl >= ns) return -1;                           // cannot happen (small_xslots bounds the count)
+        slot_rec[sl] = rec;
+        return sl;
+    };
     // The analytic cells of a step (two ghost layers of every SOURCE side, (41) / (43) / piston at t_n) are evaluated ONE STEP
     // AHEAD -- t_{n+1} = t_n + dt_n is known when step n starts, PAPER.md:279 -- by the clock warp, which idles during the
     // sweeps, each CTA the records it stores; the sweeps and the source step only load them.
     auto make_records = [&](int buf, double t, int who, int nthreads) {
         const DistRecords R{src_mem + 3 * cap_src * buf, cap_src, logc};
-        for (int sd = 0; sd < 4; ++sd) {                   // only the records of SOURCE sides exist for the readers
+        for (int sd = 2; sd < 4; ++sd) {                   // y sides; only the records of SOURCE sides exist for the readers
             if (g.side[sd].kind != BC_SOURCE) continue;
             const int first = (int)(src_off(nx, ny, sd) / 3), cnt = (int)(src_side_doubles(nx, ny, sd) / 3);
             const int per = sd < 2 ? ny + 6 : nx;          // records per ghost layer (layout of Grid::src, fvnl_bc.cuh)
@@ -319,10 +336,21 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
             }
         }
     };
-    if (tid == 0) { ck[0] = *clk; part[0].sx = part[0].sy = part[1].sx = part[1].sy = 0ull; part[0].flags = part[1].flags = 0; }
+    // ... and the x sides' in the CTA that reads them (its slots), so that the edge tile's loads stay in its own shared memory
+    auto make_xslots = [&](int buf, double t, int who, int nthreads) {
+        double* xs = xs_mem + 3 * ns * buf;
+        const int first1 = (int)(src_off(nx, ny, 1) / 3);
+        for (int sl = who; sl < nslots; sl += nthreads) {
+            const int m = slot_rec[sl], sd = m >= first1 ? 1 : 0, r = m - (sd ? first1 : 0);
+            const int layer = r / (ny + 6), pos = r - layer * (ny + 6);
+            Q3 c;
+            if (!source_at(g, sd, sd == SIDE_XLO ? -1 - layer : nx + layer, pos - 3, t, c)) { c.q1 = -1.0; c.q2 = c.q3 = 0.0; }
+            xs[sl] = c.q1; xs[ns + sl] = c.q2; xs[2 * ns + sl] = c.q3;
+        }
+    };
+    if (tid == 0) { nslots = 0; ck[0] = *clk; part[0].sx = part[0].sy = part[1].sx = part[1].sy = 0ull; part[0].flags = part[1].flags = 0; }
     __syncthreads();                                       // (ck[0])
     if (!clock_warp) {
-        if (has_src) make_records(0, ck[0].t, tid, SMALL_THREADS);
         for (int k = 0; k < rounds; ++k) {
             const int m = tile_cell(A, tx, ty, ny, k * SMALL_THREADS + tid);
             if (m >= 0) {
@@ -335,7 +363,7 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
         for (int k = 0; k < rounds; ++k) {                 // the source step's cells (same choices as source_step_cell)
             const int m = tile_cell(A, tx, ty, ny, k * SMALL_THREADS + tid);
             SrcCell c;
-            c.own = -1; c.w = c.e = c.s = c.n = 0u; c.i = c.j = 0; c.edge = 0; c.pad = 0;
+            c.own = -1; c.w = c.e = c.s = c.n = 0u; c.i = c.j = 0; c.edge = 0; c.xslot = -1;
             if (m >= 0) {
                 const int j = m / nx, i = m - j * nx;
                 const bool xlo = i == 0, xhi = i == nx - 1, ylo = j == 0, yhi = j == ny - 1;
@@ -346,6 +374,8 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
                 c.n = B.code(yhi ? (py ? 0 : j) : j + 1, i);
                 c.i = (short)i; c.j = (short)j;
                 c.edge = (xlo ? 1 : 0) | (xhi ? 2 : 0) | (ylo ? 4 : 0) | (yhi ? 8 : 0);
+                const int sd = xlo ? SIDE_XLO : SIDE_XHI;
+                if ((xlo || xhi) && g.side[sd].kind == BC_SOURCE) c.xslot = new_slot((int)src_record_index(nx, ny, sd, 0, j));
             }
             stab[k * SMALL_THREADS + tid] = c;
         }
@@ -354,16 +384,29 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
             if (m >= 0) {
                 const int row = m / nx, i = m - row * nx;
 #pragma unroll
-                for (int e = 0; e < 5; ++e) stencil[(k * 5 + e) * SMALL_THREADS + tid] = resolve_cell(g, A, i - 2 + e, row - 2);
+                for (int e = 0; e < 5; ++e) {
+                    StencilCell c = resolve_cell(g, A, i - 2 + e, row - 2);
+                    if (c.xrec >= 0) c.xrec = new_slot(c.xrec);
+                    stencil[(k * 5 + e) * SMALL_THREADS + tid] = c;
+                }
             }
         }
+    }
+    __syncthreads();                                       // (the slots are allocated)
+    if (has_src && !clock_warp) {                          // the analytic cells of the first step
+        make_records(0, ck[0].t, tid, SMALL_THREADS);
+        make_xslots(0, ck[0].t, tid, SMALL_THREADS);
     }
     cl.sync();
     for (long long step = 0; step < nsteps; ++step) {
         SmallPartial* mine = &part[step & 1];
         const Clock& now = ck[step & 1];
         const DistRecords SRC{src_mem + 3 * cap_src * (int)(step & 1), cap_src, logc};
-        if (clock_warp && has_src && step + 1 < nsteps) make_records((int)((step + 1) & 1), __dadd_rn(now.t, now.dt), lane, 32);
+        const double* xs = xs_mem + 3 * ns * (int)(step & 1);
+        if (clock_warp && has_src && step + 1 < nsteps) {
+            make_xslots((int)((step + 1) & 1), __dadd_rn(now.t, now.dt), lane, 32);
+            make_records((int)((step + 1) & 1), __dadd_rn(now.t, now.dt), lane, 32);
+        }
         if (!clock_warp) {                                 // ---- x-sweep (24) on the y-extended mesh
             const double lamx = now.lamx;
             int flags = 0;
@@ -372,7 +415,7 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
                 const int m = tile_cell(S, tx, ty, ny + 4, k * SMALL_THREADS + tid);
                 if (m < 0) continue;
                 Q3 v[5];
-                load_stencil(stencil + (size_t)k * 5 * SMALL_THREADS + tid, SMALL_THREADS, cap, SRC, v);
+                load_stencil(stencil + (size_t)k * 5 * SMALL_THREADS + tid, SMALL_THREADS, cap, SRC, xs, ns, v);
                 const int row = fdiv(m, S.inv_nx);
                 xsweep_stencil(g, lamx, v, S, m - row * nx, row - 2, sx, flags);
             }
@@ -404,13 +447,15 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
         cluster_sync_shared();
         if (!clock_warp) {                                 // ---- source step (26)
             const double kapx = now.kapx, kapy = now.kapy;
-            auto ghost = [&](int sd, const Q3& inner, int gi, int gr) {         // ghost_of, analytic cells from the records
+            auto ghost = [&](int sd, const Q3& inner, int pos, int xslot) {     // ghost_of, analytic cells from the records
                 const int kind = g.side[sd].kind;
                 Q3 c = inner;
                 if (kind == BC_REFLECT) {
                     if (sd < 2) c.q2 = -c.q2; else c.q3 = -c.q3;
                 } else if (kind == BC_SOURCE) {
-                    const Q3 a = SRC(src_record_index(nx, ny, sd, 0, sd < 2 ? gr : gi));
+                    Q3 a;
+                    if (sd < 2) { a.q1 = xs[xslot]; a.q2 = xs[ns + xslot]; a.q3 = xs[2 * ns + xslot]; }
+                    else a = SRC(src_record_index(nx, ny, sd, 0, pos));
                     if (a.q1 > 0.0) c = a;
                 }
                 return c;
@@ -423,10 +468,10 @@ __global__ void __launch_bounds__(SMALL_THREADS + 32) k_steps_cluster(Grid g, Cl
                 c.q1 = pc[0]; c.q2 = pc[cap]; c.q3 = pc[2 * cap];
                 Q3 w = B.by_code(sc.w), e = B.by_code(sc.e), s = B.by_code(sc.s), n = B.by_code(sc.n);
                 if (sc.edge) {
-                    if (sc.edge & 1) w = ghost(SIDE_XLO, w, -1, sc.j);
-                    if (sc.edge & 2) e = ghost(SIDE_XHI, e, nx, sc.j);
+                    if (sc.edge & 1) w = ghost(SIDE_XLO, w, sc.j, sc.xslot);
+                    if (sc.edge & 2) e = ghost(SIDE_XHI, e, sc.j, sc.xslot);
                     if (sc.edge & 4) s = ghost(SIDE_YLO, s, sc.i, -1);
-                    if (sc.edge & 8) n = ghost(SIDE_YHI, n, sc.i, ny);
+                    if (sc.edge & 8) n = ghost(SIDE_YHI, n, sc.i, -1);
                 }
                 const Q3 o = source_step_values(c, w, e, s, n, kapx, kapy);
                 double* pa = A.base + sc.own;
