@@ -245,9 +245,10 @@ def run_gpu(args):
     s.set_state(*q0)
     del q0
     torch.cuda.empty_cache()
-    # per-launch event pairs for the roofline; not on launch-bound grids (<= 2^18 cells), where a step is a few microseconds,
-    # the library replays CUDA graphs and an event pair per launch would be the larger part of what is measured
-    per_kernel = w.cells > (1 << 18)
+    # per-launch event pairs for the roofline; not on grids of at most 2^22 cells, where a step takes 5 ... 130 microseconds and
+    # an event pair per launch (it also keeps consecutive launches from overlapping) costs up to 10 microseconds of it -- measured
+    # on C2: 61 us per step with the pairs, 50 without: there the step IS the launch and the kernel time is ms / K
+    per_kernel = w.cells > (1 << 22)
     s.set_option(P.OPT_KERNEL_TIMING, 1 if per_kernel else 0)
 
     def barrier():

@@ -466,14 +466,21 @@ static void launch_step(fvnl_ctx* c, char** a, char** b, double value, int mode,
         const int per_sm = c->prec == 64 ? WsBudget<double>::blocks_per_sm : WsBudget<float>::blocks_per_sm;
         const int rows = fused_rows(c, strips, 148 * per_sm, 9);
         const dim3 grd(strips, (g.ny + rows - 1) / rows);
+        // programmatic dependent launch: the grid may be scheduled while the previous step's is still running; it waits for
+        // that grid's completion itself (griddepcontrol.wait in the kernel) before it touches global memory
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grd; cfg.blockDim = dim3(256); cfg.stream = c->stream;
+        cfg.dynamicSmemBytes = c->prec == 64 ? ws_smem_bytes<double>() : ws_smem_bytes<float>();
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
         if (c->prec == 64)
-            k_step_ws<double><<<grd, 256, ws_smem_bytes<double>(), c->stream>>>(
-                g, c->clk, (const double*)a[0], (const double*)a[1], (const double*)a[2], (double*)b[0], (double*)b[1],
-                (double*)b[2], rows, value, mode, more);
+            cudaLaunchKernelEx(&cfg, k_step_ws<double>, g, c->clk, (const double*)a[0], (const double*)a[1], (const double*)a[2],
+                               (double*)b[0], (double*)b[1], (double*)b[2], rows, value, mode, more);
         else
-            k_step_ws<float><<<grd, 256, ws_smem_bytes<float>(), c->stream>>>(
-                g, c->clk, (const float*)a[0], (const float*)a[1], (const float*)a[2], (float*)b[0], (float*)b[1],
-                (float*)b[2], rows, value, mode, more);
+            cudaLaunchKernelEx(&cfg, k_step_ws<float>, g, c->clk, (const float*)a[0], (const float*)a[1], (const float*)a[2],
+                               (float*)b[0], (float*)b[1], (float*)b[2], rows, value, mode, more);
     } else {
         const int strips = (g.nx + (FUSED_BX - 6) - 1) / (FUSED_BX - 6);
         const int rows = fused_rows(c, strips, 148 * FUSED_MINB);

@@ -317,7 +317,11 @@ k_step_ws(Grid g, Clock* clk, const T* __restrict__ q1, const T* __restrict__ q2
           T* __restrict__ o1, T* __restrict__ o2, T* __restrict__ o3, int rows, double value, int mode, int more) {
     extern __shared__ __align__(16) char smem[];
     const int tid = threadIdx.x;
+    // Programmatic dependent launch: let the NEXT step's grid be scheduled as this one's blocks retire, and do everything that
+    // needs no global memory (this fill) before waiting for the previous step's grid to complete and flush (its state, the clock).
+    asm volatile("griddepcontrol.launch_dependents;");
     for (int j = tid; j < ws_smem_bytes<T>() / (int)sizeof(T); j += 256) reinterpret_cast<T*>(smem)[j] = T(1);   // finite fill
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 
     StepKT<T> k;
     k.t = clk->t; k.lamx = T(clk->lamx); k.lamy = T(clk->lamy); k.kapx = T(clk->kapx); k.kapy = T(clk->kapy);
